@@ -1,0 +1,561 @@
+// api.cu -- the C ABI of libgpuann.so (include/gpuann.h): argument validation, context, weight / thermo
+// packing, the chunk loop of the tensor path.  Every step of the hot path runs in the kernels of k_*.cu.
+#include <cmath>
+#include <cstring>
+#include <new>
+
+#include "common.cuh"
+
+using namespace gpuann;
+
+struct gpuann_ctx : public Ctx {};
+
+namespace {
+
+thread_local std::string g_create_err;
+
+int fail(Ctx *c, int status, const std::string &msg) {
+    if (c) c->err = msg;
+    else g_create_err = msg;
+    return status;
+}
+
+int fail_cuda(Ctx *c, cudaError_t e, const char *what) {
+    cudaGetLastError();  // clear the sticky-less error state
+    return fail(c, e == cudaErrorMemoryAllocation ? GPUANN_ERR_ALLOC : GPUANN_ERR_CUDA,
+                std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+#define CU_TRY(ctx, call, what)                                   \
+    do {                                                          \
+        cudaError_t e__ = (call);                                 \
+        if (e__ != cudaSuccess) return fail_cuda(ctx, e__, what); \
+    } while (0)
+
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = true;
+    explicit DeviceGuard(int dev) {
+        if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+        if (prev != dev) ok = cudaSetDevice(dev) == cudaSuccess;
+    }
+    ~DeviceGuard() {
+        int cur = -1;
+        if (prev >= 0 && cudaGetDevice(&cur) == cudaSuccess && cur != prev) cudaSetDevice(prev);
+    }
+};
+
+inline int pad16(int x) { return (x + 15) / 16 * 16; }
+
+// FP32 -> BF16 bits, round to nearest even (NaN stays NaN)
+inline uint16_t f32_to_bf16_rne(float f) {
+    uint32_t u;
+    std::memcpy(&u, &f, 4);
+    if ((u & 0x7F800000u) == 0x7F800000u && (u & 0x007FFFFFu)) return (uint16_t)((u >> 16) | 0x0040u);
+    u += 0x7FFFu + ((u >> 16) & 1u);
+    return (uint16_t)(u >> 16);
+}
+
+void free_net(Ctx *c) {
+    cudaFree(c->w32);
+    cudaFree(c->b32);
+    c->w32 = c->b32 = nullptr;
+    c->w32_count = c->b32_count = 0;
+    for (int l = 0; l < kMaxLayers; ++l) {
+        cudaFree(c->lay[l].W);
+        cudaFree(c->lay[l].bias);
+        c->lay[l] = LayerBf16{};
+    }
+    cudaFree(c->act[0]);
+    cudaFree(c->act[1]);
+    cudaFree(c->o_buf);
+    c->act[0] = c->act[1] = nullptr;
+    c->o_buf = nullptr;
+    c->act_elems = 0;
+    c->net_loaded = false;
+    c->variant = "none";
+    c->issued_mac_per_cell = 0;
+}
+
+bool finite_f(float x) { return std::isfinite(x); }
+
+}  // namespace
+
+extern "C" {
+
+void gpuann_default_params(gpuann_params *p) {
+    if (!p) return;
+    p->precision = GPUANN_PRECISION_BF16;
+    p->newton_max_iter = 20;
+    p->newton_tol = 1e-6;
+    p->T_min = 200.0;
+    p->T_max = 3500.0;
+    p->T_active = 0.0;
+    p->device = -1;
+    p->chunk_cells = 0;
+}
+
+int gpuann_create(const gpuann_params *params, gpuann_ctx **out) {
+    if (!out) return fail(nullptr, GPUANN_ERR_INVALID_ARG, "gpuann_create: out is NULL");
+    *out = nullptr;
+    gpuann_params prm;
+    gpuann_default_params(&prm);
+    if (params) prm = *params;
+    if (prm.precision != GPUANN_PRECISION_FP32 && prm.precision != GPUANN_PRECISION_BF16)
+        return fail(nullptr, GPUANN_ERR_INVALID_ARG, "gpuann_create: precision must be 0 (FP32) or 1 (BF16)");
+    if (prm.newton_max_iter < 0 || !(prm.newton_tol > 0.0) || !(prm.T_min > 0.0) || !(prm.T_max > prm.T_min) ||
+        !std::isfinite(prm.T_active))
+        return fail(nullptr, GPUANN_ERR_INVALID_ARG,
+                    "gpuann_create: need newton_max_iter >= 0, newton_tol > 0, 0 < T_min < T_max, finite T_active");
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev <= 0) {
+        cudaGetLastError();
+        return fail(nullptr, GPUANN_ERR_UNSUPPORTED,
+                    std::string("gpuann_create: no CUDA device (there is no CPU fallback): ") + cudaGetErrorString(e));
+    }
+    int dev = prm.device;
+    if (dev < 0) {
+        if (cudaGetDevice(&dev) != cudaSuccess) dev = 0;
+    }
+    if (dev >= ndev) return fail(nullptr, GPUANN_ERR_INVALID_ARG, "gpuann_create: device ordinal out of range");
+    cudaDeviceProp prop;
+    if ((e = cudaGetDeviceProperties(&prop, dev)) != cudaSuccess) return fail_cuda(nullptr, e, "cudaGetDeviceProperties");
+    if (prop.major != 10)
+        return fail(nullptr, GPUANN_ERR_UNSUPPORTED,
+                    "gpuann_create: device compute capability " + std::to_string(prop.major) + "." +
+                        std::to_string(prop.minor) + " is not 10.x (this library is sm_100a only)");
+    gpuann_ctx *c = new (std::nothrow) gpuann_ctx();
+    if (!c) return fail(nullptr, GPUANN_ERR_ALLOC, "gpuann_create: host allocation failed");
+    c->prm = prm;
+    c->device = dev;
+    c->sm_count = prop.multiProcessorCount;
+    DeviceGuard g(dev);
+    if (!g.ok) {
+        delete c;
+        return fail(nullptr, GPUANN_ERR_CUDA, "gpuann_create: cudaSetDevice failed");
+    }
+    e = cudaMalloc(&c->counters, sizeof(Counters));
+    if (e == cudaSuccess) e = cudaMemset(c->counters, 0, sizeof(Counters));
+    if (e == cudaSuccess) e = cudaMalloc(&c->n_active_dev, sizeof(int32_t));
+    if (e == cudaSuccess) e = cudaMemset(c->n_active_dev, 0, sizeof(int32_t));
+    if (e == cudaSuccess) e = cudaMalloc(&c->thermo_dev, sizeof(ThermoDev));
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->own_stream, cudaStreamNonBlocking);
+    if (e == cudaSuccess && prm.precision == GPUANN_PRECISION_BF16) e = gemm_setup(c);
+    if (e != cudaSuccess) {
+        int rc = fail_cuda(nullptr, e, "gpuann_create");
+        gpuann_destroy(c);
+        return rc;
+    }
+    *out = c;
+    return GPUANN_OK;
+}
+
+int gpuann_load_net(gpuann_ctx *c, int n_species, int n_layers, const int *sizes, const float *const *weights,
+                    const float *const *biases, const float *in_mean, const float *in_std, const float *out_mean,
+                    const float *out_std, double lambda) {
+    if (!c) return fail(nullptr, GPUANN_ERR_INVALID_ARG, "gpuann_load_net: ctx is NULL");
+    if (!sizes || !weights || !biases || !in_mean || !in_std || !out_mean || !out_std)
+        return fail(c, GPUANN_ERR_INVALID_ARG, "gpuann_load_net: NULL argument");
+    if (n_species < 1 || n_layers < 1) return fail(c, GPUANN_ERR_INVALID_ARG, "gpuann_load_net: n_species, n_layers must be >= 1");
+    if (n_species > GPUANN_MAX_SPECIES || n_layers > GPUANN_MAX_LAYERS)
+        return fail(c, GPUANN_ERR_UNSUPPORTED, "gpuann_load_net: n_species > 64 or n_layers > 8");
+    if (sizes[0] != n_species + 2 || sizes[n_layers] != n_species)
+        return fail(c, GPUANN_ERR_INVALID_ARG, "gpuann_load_net: sizes[0] must be 2+Ns and sizes[L] must be Ns");
+    int maxw = 0;
+    for (int l = 0; l <= n_layers; ++l) {
+        if (sizes[l] < 1) return fail(c, GPUANN_ERR_INVALID_ARG, "gpuann_load_net: layer width < 1");
+        if (sizes[l] > GPUANN_MAX_WIDTH) return fail(c, GPUANN_ERR_UNSUPPORTED, "gpuann_load_net: layer width > 4096");
+        maxw = sizes[l] > maxw ? sizes[l] : maxw;
+    }
+    for (int l = 0; l < n_layers; ++l)
+        if (!weights[l] || !biases[l]) return fail(c, GPUANN_ERR_INVALID_ARG, "gpuann_load_net: NULL weight or bias pointer");
+    for (int j = 0; j < n_species + 2; ++j)
+        if (!finite_f(in_mean[j]) || !finite_f(in_std[j]) || !(in_std[j] > 0.f))
+            return fail(c, GPUANN_ERR_INVALID_ARG, "gpuann_load_net: in_mean must be finite and in_std finite and > 0");
+    for (int k = 0; k < n_species; ++k)
+        if (!finite_f(out_mean[k]) || !finite_f(out_std[k]))
+            return fail(c, GPUANN_ERR_INVALID_ARG, "gpuann_load_net: out_mean / out_std must be finite");
+    if (!(lambda >= 0.0) || !std::isfinite(lambda)) return fail(c, GPUANN_ERR_INVALID_ARG, "gpuann_load_net: lambda must be >= 0");
+    if (c->thermo_loaded && c->thermo_Ns != n_species)
+        return fail(c, GPUANN_ERR_INVALID_ARG, "gpuann_load_net: n_species differs from the loaded thermo table");
+
+    DeviceGuard g(c->device);
+    cudaDeviceSynchronize();
+    free_net(c);
+    c->Ns = n_species;
+    c->L = n_layers;
+    for (int l = 0; l <= n_layers; ++l) c->sizes[l] = sizes[l];
+    c->max_width = maxw;
+    c->lambda = lambda;
+
+    PreParams &pre = c->pre;
+    pre = PreParams{};
+    pre.n_species = n_species;
+    pre.lambda_zero = lambda == 0.0 ? 1 : 0;
+    pre.lambda = (float)lambda;
+    pre.inv_lambda = lambda == 0.0 ? 0.f : (float)(1.0 / lambda);
+    for (int j = 0; j < n_species + 2; ++j) {
+        pre.mean[j] = in_mean[j];
+        pre.inv_std[j] = (float)(1.0 / (double)in_std[j]);
+    }
+    PostParams &po = c->post;
+    po = PostParams{};
+    po.n_species = n_species;
+    po.newton_max_iter = c->prm.newton_max_iter;
+    po.newton_tol = c->prm.newton_tol;
+    po.T_min = c->prm.T_min;
+    po.T_max = c->prm.T_max;
+    po.lambda = lambda;
+    po.lambda_zero = pre.lambda_zero;
+    po.inv_lambda = lambda == 0.0 ? 0.0 : 1.0 / lambda;
+    po.inv_lambda_int = 0;
+    if (lambda > 0.0) {
+        const double r = std::round(po.inv_lambda);
+        if (r >= 1.0 && r <= 1024.0 && std::fabs(po.inv_lambda - r) < 1e-12 * r) po.inv_lambda_int = (int)r;
+    }
+    for (int k = 0; k < n_species; ++k) {
+        po.out_mean[k] = out_mean[k];
+        po.out_std[k] = out_std[k];
+    }
+
+    if (c->prm.precision == GPUANN_PRECISION_FP32) {
+        size_t wc = 0, bc = 0;
+        for (int l = 0; l < n_layers; ++l) {
+            wc += (size_t)sizes[l] * sizes[l + 1];
+            bc += (size_t)sizes[l + 1];
+        }
+        c->w32_count = wc;
+        c->b32_count = bc;
+        int cb = 0;
+        fp32_smem_bytes(c, &cb);
+        if (cb == 0) return fail(c, GPUANN_ERR_UNSUPPORTED, "gpuann_load_net: layer too wide for the FP32 path (max width 3200)");
+        std::vector<float> hw(wc), hb(bc);
+        size_t wo = 0, bo = 0;
+        for (int l = 0; l < n_layers; ++l) {
+            const size_t cnt = (size_t)sizes[l] * sizes[l + 1];
+            std::memcpy(hw.data() + wo, weights[l], cnt * sizeof(float));
+            std::memcpy(hb.data() + bo, biases[l], (size_t)sizes[l + 1] * sizeof(float));
+            wo += cnt;
+            bo += sizes[l + 1];
+        }
+        CU_TRY(c, cudaMalloc(&c->w32, wc * sizeof(float)), "cudaMalloc(weights)");
+        CU_TRY(c, cudaMalloc(&c->b32, bc * sizeof(float)), "cudaMalloc(biases)");
+        CU_TRY(c, cudaMemcpy(c->w32, hw.data(), wc * sizeof(float), cudaMemcpyHostToDevice), "cudaMemcpy(weights)");
+        CU_TRY(c, cudaMemcpy(c->b32, hb.data(), bc * sizeof(float), cudaMemcpyHostToDevice), "cudaMemcpy(biases)");
+        c->variant = "fp32";
+        c->issued_mac_per_cell = 0;
+        c->net_loaded = true;
+        return GPUANN_OK;
+    }
+
+    // ---- BF16 tensor path: pad, round (RNE), upload, encode the tensor maps
+    int64_t chunk = c->prm.chunk_cells > 0 ? c->prm.chunk_cells : (int64_t)c->sm_count * 128;
+    chunk = (chunk + 127) / 128 * 128;
+    c->chunk = chunk;
+    int maxKp = 0;
+    int64_t mac = 0;
+    for (int l = 0; l < n_layers; ++l) {
+        LayerBf16 &ly = c->lay[l];
+        ly.K = sizes[l];
+        ly.N = sizes[l + 1];
+        ly.Kp = pad16(ly.K);
+        ly.Np = pad16(ly.N);
+        ly.tiles_n = (ly.Np + 255) / 256;
+        ly.n_tile = pad16((ly.Np + ly.tiles_n - 1) / ly.tiles_n);
+        ly.tiles_n = (ly.Np + ly.n_tile - 1) / ly.n_tile;
+        maxKp = ly.Kp > maxKp ? ly.Kp : maxKp;
+        mac += (int64_t)ly.Kp * ly.Np;
+        std::vector<uint16_t> hw((size_t)ly.Np * ly.Kp, 0);
+        std::vector<float> hb((size_t)ly.Np, 0.f);
+        for (int j = 0; j < ly.N; ++j) {
+            for (int i = 0; i < ly.K; ++i) hw[(size_t)j * ly.Kp + i] = f32_to_bf16_rne(weights[l][(size_t)j * ly.K + i]);
+            hb[j] = biases[l][j];
+        }
+        CU_TRY(c, cudaMalloc(&ly.W, hw.size() * sizeof(uint16_t)), "cudaMalloc(W bf16)");
+        CU_TRY(c, cudaMalloc(&ly.bias, hb.size() * sizeof(float)), "cudaMalloc(bias)");
+        CU_TRY(c, cudaMemcpy(ly.W, hw.data(), hw.size() * sizeof(uint16_t), cudaMemcpyHostToDevice), "cudaMemcpy(W)");
+        CU_TRY(c, cudaMemcpy(ly.bias, hb.data(), hb.size() * sizeof(float), cudaMemcpyHostToDevice), "cudaMemcpy(bias)");
+        std::string terr;
+        if (!encode_tmap_bf16(&ly.tmapW, ly.W, (uint64_t)ly.Kp, (uint64_t)ly.Np, (uint64_t)ly.Kp * 2, (uint32_t)ly.n_tile, &terr))
+            return fail(c, GPUANN_ERR_CUDA, "gpuann_load_net: " + terr);
+    }
+    c->act_elems = (size_t)chunk * (size_t)maxKp;
+    for (int b = 0; b < 2; ++b) {
+        CU_TRY(c, cudaMalloc(&c->act[b], c->act_elems * sizeof(__nv_bfloat16)), "cudaMalloc(activations)");
+        CU_TRY(c, cudaMemset(c->act[b], 0, c->act_elems * sizeof(__nv_bfloat16)), "cudaMemset(activations)");
+    }
+    CU_TRY(c, cudaMalloc(&c->o_buf, (size_t)n_species * chunk * sizeof(float)), "cudaMalloc(o_buf)");
+    CU_TRY(c, cudaMemset(c->o_buf, 0, (size_t)n_species * chunk * sizeof(float)), "cudaMemset(o_buf)");
+    for (int l = 0; l < n_layers; ++l) {
+        LayerBf16 &ly = c->lay[l];
+        std::string terr;
+        if (!encode_tmap_bf16(&ly.tmapA, c->act[l & 1], (uint64_t)ly.Kp, (uint64_t)chunk, (uint64_t)ly.Kp * 2, 128, &terr))
+            return fail(c, GPUANN_ERR_CUDA, "gpuann_load_net: " + terr);
+    }
+    c->issued_mac_per_cell = mac;
+    c->variant = "bf16-layerwise";
+    c->net_loaded = true;
+    return GPUANN_OK;
+}
+
+int gpuann_load_thermo(gpuann_ctx *c, int n_species, const double *nasa_lo, const double *nasa_hi, const double *T_mid,
+                       const double *W) {
+    if (!c) return fail(nullptr, GPUANN_ERR_INVALID_ARG, "gpuann_load_thermo: ctx is NULL");
+    if (!nasa_lo || !W) return fail(c, GPUANN_ERR_INVALID_ARG, "gpuann_load_thermo: nasa_lo or W is NULL");
+    if (n_species < 1) return fail(c, GPUANN_ERR_INVALID_ARG, "gpuann_load_thermo: n_species < 1");
+    if (n_species > GPUANN_MAX_SPECIES) return fail(c, GPUANN_ERR_UNSUPPORTED, "gpuann_load_thermo: n_species > 64");
+    if (c->net_loaded && c->Ns != n_species)
+        return fail(c, GPUANN_ERR_INVALID_ARG, "gpuann_load_thermo: n_species differs from the loaded net");
+    const bool two = nasa_hi && T_mid;
+    ThermoDev *h = new (std::nothrow) ThermoDev();
+    if (!h) return fail(c, GPUANN_ERR_ALLOC, "gpuann_load_thermo: host allocation failed");
+    std::memset(h, 0, sizeof(ThermoDev));
+    h->n_species = n_species;
+    h->two_ranges = two ? 1 : 0;
+    for (int k = 0; k < n_species; ++k) {
+        if (!(W[k] > 0.0) || !std::isfinite(W[k])) {
+            delete h;
+            return fail(c, GPUANN_ERR_INVALID_ARG, "gpuann_load_thermo: W must be finite and > 0");
+        }
+        const double s = kRu / W[k];
+        for (int r = 0; r < 2; ++r) {
+            const double *a = (r == 1 && two) ? nasa_hi + 7 * k : nasa_lo + 7 * k;
+            for (int j = 0; j < 7; ++j)
+                if (!std::isfinite(a[j])) {
+                    delete h;
+                    return fail(c, GPUANN_ERR_INVALID_ARG, "gpuann_load_thermo: non-finite NASA-7 coefficient");
+                }
+            for (int j = 0; j < 5; ++j) h->cp[k][r][j] = s * a[j];
+            h->hh[k][r][0] = s * a[5];
+            h->hh[k][r][1] = s * a[0];
+            h->hh[k][r][2] = s * a[1] / 2.0;
+            h->hh[k][r][3] = s * a[2] / 3.0;
+            h->hh[k][r][4] = s * a[3] / 4.0;
+            h->hh[k][r][5] = s * a[4] / 5.0;
+        }
+        h->T_mid[k] = two ? T_mid[k] : 0.0;
+    }
+    DeviceGuard g(c->device);
+    cudaDeviceSynchronize();
+    cudaError_t e = cudaMemcpy(c->thermo_dev, h, sizeof(ThermoDev), cudaMemcpyHostToDevice);
+    delete h;
+    if (e != cudaSuccess) return fail_cuda(c, e, "gpuann_load_thermo: cudaMemcpy");
+    c->thermo_loaded = true;
+    c->thermo_Ns = n_species;
+    return GPUANN_OK;
+}
+
+}  // extern "C"
+
+// ================================================================ the step
+namespace {
+
+int ensure_compaction_scratch(Ctx *c, int64_t n) {
+    if (n > c->idx_cap) {
+        cudaFree(c->idx);
+        c->idx = nullptr;
+        c->idx_cap = 0;
+        CU_TRY(c, cudaMalloc(&c->idx, (size_t)n * sizeof(int32_t)), "cudaMalloc(idx)");
+        c->idx_cap = n;
+    }
+    const int64_t nb = (n + 2047) / 2048;
+    if (nb > c->blk_cap) {
+        cudaFree(c->blk_counts);
+        c->blk_counts = nullptr;
+        c->blk_cap = 0;
+        CU_TRY(c, cudaMalloc(&c->blk_counts, (size_t)nb * sizeof(int32_t)), "cudaMalloc(blk_counts)");
+        c->blk_cap = nb;
+    }
+    return GPUANN_OK;
+}
+
+// S1-S3 of the tensor path for the chunk [c0, c0+cn): z -> layers -> raw output o (FP32, [Ns][stride])
+int forward_chunk_bf16(Ctx *c, int64_t n, int64_t c0, int64_t cn, const float *T, const float *p, const float *Y,
+                       bool use_idx, float *o, int64_t o_stride, cudaStream_t s) {
+    CU_TRY(c, launch_pre_bf16(c, n, c0, cn, T, p, Y, use_idx, c->act[0], c->lay[0].Kp, s), "pre kernel");
+    for (int l = 0; l < c->L; ++l) {
+        const bool last = l == c->L - 1;
+        __nv_bfloat16 *out = last ? nullptr : c->act[(l + 1) & 1];
+        CU_TRY(c,
+               launch_layer_bf16(c, l, cn, &c->lay[l].tmapA, out, last ? 0 : c->lay[l + 1].Kp, last ? o : nullptr,
+                                 o_stride, c0, use_idx, s),
+               "layer kernel");
+    }
+    return GPUANN_OK;
+}
+
+int check_step_args(Ctx *c, const char *fn, int64_t n, const void *T, const void *p, const void *Y, const void *h,
+                    double dt, bool need_thermo) {
+    if (n < 0) return fail(c, GPUANN_ERR_INVALID_ARG, std::string(fn) + ": n_cells < 0");
+    if (n > 0 && (!T || !p || !Y || (need_thermo && !h))) return fail(c, GPUANN_ERR_INVALID_ARG, std::string(fn) + ": NULL state pointer");
+    if (need_thermo && (!(dt > 0.0) || !std::isfinite(dt))) return fail(c, GPUANN_ERR_INVALID_ARG, std::string(fn) + ": dt must be > 0");
+    if (n > 0x7FFFFFFFLL) return fail(c, GPUANN_ERR_UNSUPPORTED, std::string(fn) + ": n_cells >= 2^31");
+    if (!c->net_loaded || (need_thermo && !c->thermo_loaded))
+        return fail(c, GPUANN_ERR_NOT_READY, std::string(fn) + ": load_net" + (need_thermo ? " and load_thermo" : "") + " first");
+    return GPUANN_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int gpuann_chem_step(gpuann_ctx *c, int64_t n, float *T, const float *p, float *Y, const float *h, double dt,
+                     void *stream) {
+    if (!c) return fail(nullptr, GPUANN_ERR_INVALID_ARG, "gpuann_chem_step: ctx is NULL");
+    int rc = check_step_args(c, "gpuann_chem_step", n, T, p, Y, h, dt, true);
+    if (rc != GPUANN_OK) return rc;
+    if (n == 0) return GPUANN_OK;
+    DeviceGuard g(c->device);
+    cudaStream_t s = reinterpret_cast<cudaStream_t>(stream);
+    c->last_stream = s;
+    if (c->prm.precision == GPUANN_PRECISION_FP32) {
+        CU_TRY(c, launch_chem_fp32(c, n, T, p, Y, h, dt, nullptr, false, s), "fp32 kernel");
+        return GPUANN_OK;
+    }
+    const bool use_idx = c->prm.T_active > 0.0;
+    if (use_idx) {
+        rc = ensure_compaction_scratch(c, n);
+        if (rc != GPUANN_OK) return rc;
+        CU_TRY(c, launch_compact(c, n, T, (float)c->prm.T_active, s), "compaction kernels");
+    } else {
+        c->host_active += n;
+    }
+    for (int64_t c0 = 0; c0 < n; c0 += c->chunk) {
+        const int64_t cn = (n - c0) < c->chunk ? (n - c0) : c->chunk;
+        rc = forward_chunk_bf16(c, n, c0, cn, T, p, Y, use_idx, c->o_buf, c->chunk, s);
+        if (rc != GPUANN_OK) return rc;
+        CU_TRY(c, launch_post(c, n, c0, cn, T, Y, h, c->o_buf, c->chunk, dt, use_idx, s), "update kernel");
+    }
+    return GPUANN_OK;
+}
+
+int gpuann_debug_forward(gpuann_ctx *c, int64_t n, const float *T, const float *p, const float *Y, float *o_raw,
+                         void *stream) {
+    if (!c) return fail(nullptr, GPUANN_ERR_INVALID_ARG, "gpuann_debug_forward: ctx is NULL");
+    int rc = check_step_args(c, "gpuann_debug_forward", n, T, p, Y, nullptr, 1.0, false);
+    if (rc != GPUANN_OK) return rc;
+    if (n > 0 && !o_raw) return fail(c, GPUANN_ERR_INVALID_ARG, "gpuann_debug_forward: o_raw is NULL");
+    if (n == 0) return GPUANN_OK;
+    DeviceGuard g(c->device);
+    cudaStream_t s = reinterpret_cast<cudaStream_t>(stream);
+    c->last_stream = s;
+    if (c->prm.precision == GPUANN_PRECISION_FP32) {
+        CU_TRY(c, launch_chem_fp32(c, n, const_cast<float *>(T), p, const_cast<float *>(Y), nullptr, 1.0, o_raw, true, s),
+               "fp32 kernel");
+        return GPUANN_OK;
+    }
+    for (int64_t c0 = 0; c0 < n; c0 += c->chunk) {
+        const int64_t cn = (n - c0) < c->chunk ? (n - c0) : c->chunk;
+        rc = forward_chunk_bf16(c, n, c0, cn, T, p, Y, false, o_raw + c0, n, s);
+        if (rc != GPUANN_OK) return rc;
+    }
+    return GPUANN_OK;
+}
+
+int gpuann_chem_step_host(gpuann_ctx *c, int64_t n, float *T, const float *p, float *Y, const float *h, double dt) {
+    if (!c) return fail(nullptr, GPUANN_ERR_INVALID_ARG, "gpuann_chem_step_host: ctx is NULL");
+    int rc = check_step_args(c, "gpuann_chem_step_host", n, T, p, Y, h, dt, true);
+    if (rc != GPUANN_OK) return rc;
+    if (n == 0) return GPUANN_OK;
+    DeviceGuard g(c->device);
+    const size_t Ns = (size_t)c->Ns;
+    const size_t need = (3 + Ns) * (size_t)n;
+    if (need > c->stage_floats) {
+        cudaFree(c->stage);
+        c->stage = nullptr;
+        c->stage_floats = 0;
+        CU_TRY(c, cudaMalloc(&c->stage, need * sizeof(float)), "cudaMalloc(staging)");
+        c->stage_floats = need;
+    }
+    float *dT = c->stage, *dp = dT + n, *dh = dp + n, *dY = dh + n;
+    cudaStream_t s = c->own_stream;
+    const size_t fb = (size_t)n * sizeof(float);
+    CU_TRY(c, cudaMemcpyAsync(dT, T, fb, cudaMemcpyHostToDevice, s), "H2D T");
+    CU_TRY(c, cudaMemcpyAsync(dp, p, fb, cudaMemcpyHostToDevice, s), "H2D p");
+    CU_TRY(c, cudaMemcpyAsync(dh, h, fb, cudaMemcpyHostToDevice, s), "H2D h");
+    CU_TRY(c, cudaMemcpyAsync(dY, Y, fb * Ns, cudaMemcpyHostToDevice, s), "H2D Y");
+    rc = gpuann_chem_step(c, n, dT, dp, dY, dh, dt, s);
+    if (rc != GPUANN_OK) return rc;
+    CU_TRY(c, cudaMemcpyAsync(T, dT, fb, cudaMemcpyDeviceToHost, s), "D2H T");
+    CU_TRY(c, cudaMemcpyAsync(Y, dY, fb * Ns, cudaMemcpyDeviceToHost, s), "D2H Y");
+    CU_TRY(c, cudaStreamSynchronize(s), "cudaStreamSynchronize");
+    return GPUANN_OK;
+}
+
+int gpuann_get_stats(gpuann_ctx *c, int64_t *n_active, int64_t *n_not_converged, int64_t *n_degenerate) {
+    if (!c) return fail(nullptr, GPUANN_ERR_INVALID_ARG, "gpuann_get_stats: ctx is NULL");
+    DeviceGuard g(c->device);
+    CU_TRY(c, cudaStreamSynchronize(c->last_stream), "cudaStreamSynchronize");
+    Counters h;
+    CU_TRY(c, cudaMemcpy(&h, c->counters, sizeof(h), cudaMemcpyDeviceToHost), "cudaMemcpy(counters)");
+    if (n_active) *n_active = (int64_t)h.n_active + c->host_active;
+    if (n_not_converged) *n_not_converged = (int64_t)h.n_not_converged;
+    if (n_degenerate) *n_degenerate = (int64_t)h.n_degenerate;
+    return GPUANN_OK;
+}
+
+int gpuann_reset_stats(gpuann_ctx *c) {
+    if (!c) return fail(nullptr, GPUANN_ERR_INVALID_ARG, "gpuann_reset_stats: ctx is NULL");
+    DeviceGuard g(c->device);
+    CU_TRY(c, cudaStreamSynchronize(c->last_stream), "cudaStreamSynchronize");
+    CU_TRY(c, cudaMemset(c->counters, 0, sizeof(Counters)), "cudaMemset(counters)");
+    c->host_active = 0;
+    return GPUANN_OK;
+}
+
+int gpuann_enthalpy(gpuann_ctx *c, int64_t n, const float *T, const float *Y, float *h_out, void *stream) {
+    if (!c) return fail(nullptr, GPUANN_ERR_INVALID_ARG, "gpuann_enthalpy: ctx is NULL");
+    if (n < 0 || (n > 0 && (!T || !Y || !h_out))) return fail(c, GPUANN_ERR_INVALID_ARG, "gpuann_enthalpy: bad argument");
+    if (!c->thermo_loaded) return fail(c, GPUANN_ERR_NOT_READY, "gpuann_enthalpy: load_thermo first");
+    DeviceGuard g(c->device);
+    cudaStream_t s = reinterpret_cast<cudaStream_t>(stream);
+    c->last_stream = s;
+    CU_TRY(c, launch_enthalpy(c, n, T, Y, h_out, s), "enthalpy kernel");
+    return GPUANN_OK;
+}
+
+int gpuann_input_moments(gpuann_ctx *c, int64_t n, int n_species, const float *T, const float *p, const float *Y,
+                         double lambda, double *mean_out, double *std_out, void *stream) {
+    if (!c) return fail(nullptr, GPUANN_ERR_INVALID_ARG, "gpuann_input_moments: ctx is NULL");
+    if (n <= 0 || n_species < 1 || n_species > GPUANN_MAX_SPECIES || !T || !p || !Y || !mean_out || !std_out ||
+        !(lambda >= 0.0))
+        return fail(c, GPUANN_ERR_INVALID_ARG, "gpuann_input_moments: bad argument");
+    DeviceGuard g(c->device);
+    cudaStream_t s = reinterpret_cast<cudaStream_t>(stream);
+    c->last_stream = s;
+    CU_TRY(c, launch_moments(c, n, n_species, T, p, Y, lambda, mean_out, std_out, s), "moments kernel");
+    return GPUANN_OK;
+}
+
+int64_t gpuann_launch_count(const gpuann_ctx *c) { return c ? c->launches : 0; }
+
+int gpuann_describe(const gpuann_ctx *c, int64_t *issued_mac_per_cell, const char **variant) {
+    if (!c) return GPUANN_ERR_INVALID_ARG;
+    if (issued_mac_per_cell) *issued_mac_per_cell = c->issued_mac_per_cell;
+    if (variant) *variant = c->variant;
+    return GPUANN_OK;
+}
+
+const char *gpuann_last_error(const gpuann_ctx *c) { return c ? c->err.c_str() : g_create_err.c_str(); }
+
+int gpuann_destroy(gpuann_ctx *c) {
+    if (!c) return GPUANN_OK;
+    {
+        DeviceGuard g(c->device);
+        cudaDeviceSynchronize();
+        free_net(c);
+        cudaFree(c->thermo_dev);
+        cudaFree(c->idx);
+        cudaFree(c->blk_counts);
+        cudaFree(c->n_active_dev);
+        cudaFree(c->stage);
+        cudaFree(c->counters);
+        if (c->own_stream) cudaStreamDestroy(c->own_stream);
+        cudaGetLastError();
+    }
+    delete c;
+    return GPUANN_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,151 @@
+// common.cuh -- internal declarations shared by the translation units of libgpuann.so
+// (context, device-side parameter blocks, launch prototypes).  Not part of the public ABI.
+#pragma once
+#include <cstdint>
+#include <cstdio>
+#include <string>
+#include <vector>
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+
+#include "../../include/gpuann.h"
+
+namespace gpuann {
+
+constexpr int kMaxSpecies = GPUANN_MAX_SPECIES;
+constexpr int kMaxLayers = GPUANN_MAX_LAYERS;
+constexpr double kRu = 8314.46261815324;  // J/(kmol K)
+
+// ---------------------------------------------------------------- device-side parameter blocks
+// Thermo table in the form the T-solve evaluates: per species and range, pre-scaled by Ru/W_k:
+//   cp_k(T) = c[0] + T (c[1] + T (c[2] + T (c[3] + T c[4])))
+//   h_k(T)  = c[5] + T (c[0] + T (c[1]/2 + T (c[2]/3 + T (c[3]/4 + T c[4]/5))))  -- the /j factors are stored in d[]
+struct ThermoDev {
+    double cp[kMaxSpecies][2][5];  // (Ru/W) a1..a5
+    double hh[kMaxSpecies][2][6];  // (Ru/W) {a6, a1, a2/2, a3/3, a4/4, a5/5}
+    double T_mid[kMaxSpecies];
+    int n_species;
+    int two_ranges;
+};
+
+// Everything the update S4-S7 needs besides the thermo table.
+struct PostParams {
+    int n_species;
+    int newton_max_iter;
+    int inv_lambda_int;  // > 0: 1/lambda is this integer (power by repeated squaring); 0: generic pow
+    int lambda_zero;     // 1: log/exp branch of Eq. 7
+    double lambda;
+    double inv_lambda;
+    double newton_tol;
+    double T_min, T_max;
+    float out_mean[kMaxSpecies];
+    float out_std[kMaxSpecies];
+};
+
+// Input side S1-S2: z_j = (x_j - mean_j) * inv_std_j
+struct PreParams {
+    int n_species;
+    int lambda_zero;
+    float lambda;
+    float inv_lambda;
+    float mean[kMaxSpecies + 2];
+    float inv_std[kMaxSpecies + 2];
+};
+
+struct Counters {
+    unsigned long long n_active;
+    unsigned long long n_not_converged;
+    unsigned long long n_degenerate;
+    unsigned long long pad;
+};
+
+// One layer of the BF16 tensor path.
+struct LayerBf16 {
+    int K, N;            // true fan-in / fan-out
+    int Kp, Np;          // padded to multiples of 16
+    int n_tile;          // UMMA N of a full tile (multiple of 16, <= 256)
+    int tiles_n;         // ceil(Np / n_tile)
+    __nv_bfloat16 *W;    // DEVICE [Np][Kp] row-major, zero padded
+    float *bias;         // DEVICE [Np], zero padded
+    CUtensorMap tmapW;   // box {64, n_tile}, SWIZZLE_128B
+    CUtensorMap tmapA;   // this layer's input: activation buffer [chunk][Kp], box {64, 128}
+};
+
+struct Ctx {
+    gpuann_params prm{};
+    int device = 0;
+    int sm_count = 0;
+    std::string err;
+
+    // net
+    bool net_loaded = false;
+    int Ns = 0, L = 0;
+    int sizes[kMaxLayers + 1]{};
+    double lambda = 0.1;
+    PreParams pre{};
+    PostParams post{};
+    // FP32 path
+    float *w32 = nullptr;        // DEVICE concatenated [out][in] per layer
+    float *b32 = nullptr;        // DEVICE concatenated
+    size_t w32_count = 0, b32_count = 0;
+    int max_width = 0;
+    // BF16 path
+    LayerBf16 lay[kMaxLayers]{};
+    int64_t chunk = 0;                        // cells per pass
+    __nv_bfloat16 *act[2] = {nullptr, nullptr};  // ping-pong activation buffers [chunk][maxKp]
+    size_t act_elems = 0;
+    float *o_buf = nullptr;                   // [Ns][chunk] raw output of the chunk
+    int64_t issued_mac_per_cell = 0;
+    const char *variant = "none";
+
+    // thermo
+    bool thermo_loaded = false;
+    int thermo_Ns = 0;
+    ThermoDev *thermo_dev = nullptr;  // DEVICE
+
+    // compaction scratch (S0)
+    int32_t *idx = nullptr;       // DEVICE [idx_cap] active cell indices
+    int64_t idx_cap = 0;
+    int32_t *blk_counts = nullptr;  // DEVICE per-block counts / offsets
+    int64_t blk_cap = 0;
+    int32_t *n_active_dev = nullptr;  // DEVICE int32: number of active cells of the current step
+
+    // host-variant staging
+    float *stage = nullptr;
+    size_t stage_floats = 0;
+
+    Counters *counters = nullptr;  // DEVICE
+    int64_t host_active = 0;       // cells counted as active without a device-side compaction
+    cudaStream_t own_stream = nullptr;  // used by gpuann_chem_step_host
+    cudaStream_t last_stream = nullptr;
+    int64_t launches = 0;
+};
+
+// ---------------------------------------------------------------- kernel launchers (defined in the .cu files)
+// k_fp32.cu
+cudaError_t launch_chem_fp32(Ctx *c, int64_t n, float *T, const float *p, float *Y, const float *h, double dt,
+                             float *o_raw, bool forward_only, cudaStream_t s);
+size_t fp32_smem_bytes(const Ctx *c, int *cells_per_block);
+
+// k_aux.cu
+cudaError_t launch_compact(Ctx *c, int64_t n, const float *T, float T_active, cudaStream_t s);
+cudaError_t launch_pre_bf16(Ctx *c, int64_t n, int64_t c0, int64_t cn, const float *T, const float *p, const float *Y,
+                            bool use_idx, __nv_bfloat16 *z, int Kp, cudaStream_t s);
+cudaError_t launch_post(Ctx *c, int64_t n, int64_t c0, int64_t cn, float *T, float *Y, const float *h, const float *o,
+                        int64_t o_stride, double dt, bool use_idx, cudaStream_t s);
+cudaError_t launch_enthalpy(Ctx *c, int64_t n, const float *T, const float *Y, float *h_out, cudaStream_t s);
+cudaError_t launch_moments(Ctx *c, int64_t n, int Ns, const float *T, const float *p, const float *Y, double lambda,
+                           double *mean_out, double *std_out, cudaStream_t s);
+
+// k_gemm.cu
+cudaError_t gemm_setup(Ctx *c);  // opt-in shared memory etc.
+cudaError_t launch_layer_bf16(Ctx *c, int layer, int64_t rows_cap, const CUtensorMap *tmapA, __nv_bfloat16 *out_bf16,
+                              int out_ld, float *out_f32, int64_t out_f32_stride, int64_t c0, bool use_count,
+                              cudaStream_t s);
+
+// encodes a 2-D BF16 row-major tensor map {inner = cols, outer = rows}, box {64, box_rows}, 128-byte swizzle
+bool encode_tmap_bf16(CUtensorMap *out, const void *base, uint64_t cols, uint64_t rows, uint64_t row_pitch_bytes,
+                      uint32_t box_rows, std::string *err);
+
+}  // namespace gpuann

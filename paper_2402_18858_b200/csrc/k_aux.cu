@@ -1,0 +1,328 @@
+// k_aux.cu -- the HBM-bound kernels around the MLP: S0 active-cell compaction, S1+S2 (Box-Cox + normalise ->
+// BF16 rows for the tensor path), S4-S7 (update + Newton T-solve) as a stand-alone kernel, and the input-recipe
+// helpers gpuann_enthalpy / gpuann_input_moments.  All state accesses are along the cell index of the SoA
+// fields, i.e. coalesced 128-byte lines per warp.
+#include "common.cuh"
+#include "post.cuh"
+
+namespace gpuann {
+
+// ================================================================ S0: compaction (BASELINE.json configs[4]; R12)
+// Order-preserving: idx[] lists the active cells in increasing cell order, so results do not depend on timing.
+constexpr int kCompThreads = 256;
+constexpr int kCompPerThread = 8;
+constexpr int kCompPerBlock = kCompThreads * kCompPerThread;
+
+__device__ __forceinline__ int block_exclusive_scan_256(int v, int *total) {
+    __shared__ int warp_sums[kCompThreads / 32];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    int incl = v;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        int t = __shfl_up_sync(0xffffffffu, incl, d);
+        if (lane >= d) incl += t;
+    }
+    if (lane == 31) warp_sums[w] = incl;
+    __syncthreads();
+    int base = 0, tot = 0;
+#pragma unroll
+    for (int i = 0; i < kCompThreads / 32; ++i) {
+        int s = warp_sums[i];
+        if (i < w) base += s;
+        tot += s;
+    }
+    __syncthreads();
+    *total = tot;
+    return base + incl - v;
+}
+
+__global__ void __launch_bounds__(kCompThreads) k_compact_count(int64_t n, const float *__restrict__ T, float T_active,
+                                                                int32_t *__restrict__ blk_counts) {
+    const int64_t base = (int64_t)blockIdx.x * kCompPerBlock + (int64_t)threadIdx.x * kCompPerThread;
+    int cnt = 0;
+#pragma unroll
+    for (int j = 0; j < kCompPerThread; ++j) {
+        const int64_t i = base + j;
+        if (i < n && !(T[i] < T_active)) ++cnt;
+    }
+    int total;
+    (void)block_exclusive_scan_256(cnt, &total);
+    if (threadIdx.x == 0) blk_counts[blockIdx.x] = total;
+}
+
+// one block: exclusive scan of the per-block counts in place; total -> *n_active and the statistics counter
+__global__ void __launch_bounds__(kCompThreads) k_compact_scan(int nb, int32_t *__restrict__ blk_counts,
+                                                               int32_t *__restrict__ n_active,
+                                                               Counters *__restrict__ counters) {
+    __shared__ int carry_s;
+    if (threadIdx.x == 0) carry_s = 0;
+    __syncthreads();
+    for (int b0 = 0; b0 < nb; b0 += kCompThreads) {
+        const int b = b0 + threadIdx.x;
+        const int v = b < nb ? blk_counts[b] : 0;
+        int total;
+        const int ex = block_exclusive_scan_256(v, &total);
+        const int carry = carry_s;
+        if (b < nb) blk_counts[b] = carry + ex;
+        __syncthreads();
+        if (threadIdx.x == 0) carry_s = carry + total;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        *n_active = carry_s;
+        counters->n_active += (unsigned long long)carry_s;
+    }
+}
+
+__global__ void __launch_bounds__(kCompThreads) k_compact_scatter(int64_t n, const float *__restrict__ T, float T_active,
+                                                                  const int32_t *__restrict__ blk_offsets,
+                                                                  int32_t *__restrict__ idx) {
+    const int64_t base = (int64_t)blockIdx.x * kCompPerBlock + (int64_t)threadIdx.x * kCompPerThread;
+    unsigned mask = 0;
+    int cnt = 0;
+#pragma unroll
+    for (int j = 0; j < kCompPerThread; ++j) {
+        const int64_t i = base + j;
+        if (i < n && !(T[i] < T_active)) {
+            mask |= 1u << j;
+            ++cnt;
+        }
+    }
+    int total;
+    int pos = blk_offsets[blockIdx.x] + block_exclusive_scan_256(cnt, &total);
+#pragma unroll
+    for (int j = 0; j < kCompPerThread; ++j)
+        if (mask & (1u << j)) idx[pos++] = (int32_t)(base + j);
+}
+
+cudaError_t launch_compact(Ctx *c, int64_t n, const float *T, float T_active, cudaStream_t s) {
+    const int nb = (int)((n + kCompPerBlock - 1) / kCompPerBlock);
+    k_compact_count<<<nb, kCompThreads, 0, s>>>(n, T, T_active, c->blk_counts);
+    k_compact_scan<<<1, kCompThreads, 0, s>>>(nb, c->blk_counts, c->n_active_dev, c->counters);
+    k_compact_scatter<<<nb, kCompThreads, 0, s>>>(n, T, T_active, c->blk_counts, c->idx);
+    c->launches += 3;
+    return cudaGetLastError();
+}
+
+// ================================================================ S1 + S2 -> BF16 rows (R1, R2, R4)
+// One thread per cell of the chunk [c0, c0+cn): z[i][0..Kp) = BF16((x_j - mean_j) * inv_std_j), x = {T, p, y_1..y_Ns},
+// zero padded to Kp columns (a multiple of 16, <= 80 here).  Row i of z is 2*Kp bytes, written as 16-byte stores.
+__global__ void __launch_bounds__(128) k_pre_bf16(int64_t n, int64_t c0, int64_t cn, const float *__restrict__ T,
+                                                  const float *__restrict__ p, const float *__restrict__ Y,
+                                                  const int32_t *__restrict__ idx, const int32_t *__restrict__ n_active,
+                                                  __nv_bfloat16 *__restrict__ z, int Kp, const PreParams pp) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= cn) return;
+    int64_t g = c0 + i;
+    bool valid = true;
+    if (idx) {
+        valid = g < (int64_t)*n_active;
+        g = valid ? (int64_t)idx[g] : 0;
+    }
+    uint4 *row = reinterpret_cast<uint4 *>(z + i * Kp);
+    const int D = pp.n_species + 2;
+    for (int j0 = 0; j0 < Kp; j0 += 8) {
+        float v[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            const int j = j0 + q;
+            float x = 0.f;
+            if (valid && j < D) {
+                if (j == 0) x = T[g];
+                else if (j == 1) x = p[g];
+                else {
+                    const float Yc = fmaxf(Y[(int64_t)(j - 2) * n + g], 0.f);
+                    x = boxcox_y(Yc, boxcox_u(Yc, pp.lambda), pp);
+                }
+                x = (x - pp.mean[j]) * pp.inv_std[j];
+            }
+            v[q] = x;
+        }
+        uint4 o;
+        __nv_bfloat162 t0 = __floats2bfloat162_rn(v[0], v[1]);
+        __nv_bfloat162 t1 = __floats2bfloat162_rn(v[2], v[3]);
+        __nv_bfloat162 t2 = __floats2bfloat162_rn(v[4], v[5]);
+        __nv_bfloat162 t3 = __floats2bfloat162_rn(v[6], v[7]);
+        o.x = *reinterpret_cast<uint32_t *>(&t0);
+        o.y = *reinterpret_cast<uint32_t *>(&t1);
+        o.z = *reinterpret_cast<uint32_t *>(&t2);
+        o.w = *reinterpret_cast<uint32_t *>(&t3);
+        row[j0 >> 3] = o;
+    }
+}
+
+cudaError_t launch_pre_bf16(Ctx *c, int64_t n, int64_t c0, int64_t cn, const float *T, const float *p, const float *Y,
+                            bool use_idx, __nv_bfloat16 *z, int Kp, cudaStream_t s) {
+    if (cn <= 0) return cudaSuccess;
+    const int blocks = (int)((cn + 127) / 128);
+    k_pre_bf16<<<blocks, 128, 0, s>>>(n, c0, cn, T, p, Y, use_idx ? c->idx : nullptr, c->n_active_dev, z, Kp, c->pre);
+    c->launches += 1;
+    return cudaGetLastError();
+}
+
+// ================================================================ S4-S7 as a stand-alone kernel
+// One thread per cell of the chunk.  o[k*o_stride + i] is the raw network output of local cell i.
+// Writes Y_new (FP32, in place) and T_new; skipped / out-of-range cells are not touched.
+__global__ void __launch_bounds__(128) k_post(int64_t n, int64_t c0, int64_t cn, float *__restrict__ T,
+                                              float *__restrict__ Y, const float *__restrict__ h,
+                                              const float *__restrict__ o, int64_t o_stride, double dt,
+                                              const int32_t *__restrict__ idx, const int32_t *__restrict__ n_active,
+                                              const ThermoDev *__restrict__ thermo_g, Counters *__restrict__ counters,
+                                              float lambda_f, const PostParams pp) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    ThermoDev *th = reinterpret_cast<ThermoDev *>(smem_raw);
+    {
+        const int words = (int)(sizeof(ThermoDev) / 4);
+        const uint32_t *src = reinterpret_cast<const uint32_t *>(thermo_g);
+        uint32_t *dst = reinterpret_cast<uint32_t *>(th);
+        for (int w = threadIdx.x; w < words; w += blockDim.x) dst[w] = src[w];
+    }
+    __syncthreads();
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int Ns = pp.n_species;
+    bool valid = i < cn;
+    int64_t g = c0 + i;
+    if (valid && idx) {
+        valid = g < (int64_t)*n_active;
+        g = valid ? (int64_t)idx[g] : 0;
+    }
+    unsigned nconv = 0, ndeg = 0;
+    if (valid) {
+        double Yc[kMaxSpecies], Ys[kMaxSpecies];
+#pragma unroll 1
+        for (int k = 0; k < Ns; ++k) {
+            const float yf = fmaxf(Y[(int64_t)k * n + g], 0.f);
+            const float u = boxcox_u(yf, lambda_f);
+            Yc[k] = (double)yf;
+            Ys[k] = update_species((double)yf, u, o[(int64_t)k * o_stride + i], pp.out_std[k], pp.out_mean[k], dt, pp);
+        }
+        if (renormalise<kMaxSpecies>(Ys, Yc, Ns)) ndeg = 1;
+        bool conv;
+        const double Tn = newton_T<kMaxSpecies>(Ys, Ns, (double)h[g], (double)T[g], th, pp, &conv);
+        if (!conv) nconv = 1;
+#pragma unroll 1
+        for (int k = 0; k < Ns; ++k) Y[(int64_t)k * n + g] = (float)Ys[k];
+        T[g] = (float)Tn;
+    }
+    // statistics: one atomic per warp and counter, only when something happened
+    nconv = __reduce_add_sync(0xffffffffu, nconv);
+    ndeg = __reduce_add_sync(0xffffffffu, ndeg);
+    if ((threadIdx.x & 31) == 0) {
+        if (nconv) atomicAdd(&counters->n_not_converged, (unsigned long long)nconv);
+        if (ndeg) atomicAdd(&counters->n_degenerate, (unsigned long long)ndeg);
+    }
+}
+
+cudaError_t launch_post(Ctx *c, int64_t n, int64_t c0, int64_t cn, float *T, float *Y, const float *h, const float *o,
+                        int64_t o_stride, double dt, bool use_idx, cudaStream_t s) {
+    if (cn <= 0) return cudaSuccess;
+    const int blocks = (int)((cn + 127) / 128);
+    k_post<<<blocks, 128, sizeof(ThermoDev), s>>>(n, c0, cn, T, Y, h, o, o_stride, dt, use_idx ? c->idx : nullptr,
+                                                   c->n_active_dev, c->thermo_dev, c->counters, (float)c->lambda,
+                                                   c->post);
+    c->launches += 1;
+    return cudaGetLastError();
+}
+
+// ================================================================ input-recipe helpers (G4, G5)
+// G5: h_i = sum_k Y[k][i] h_k(T_i) in FP64 from the FP32 state, rounded to FP32.
+__global__ void __launch_bounds__(128) k_enthalpy(int64_t n, const float *__restrict__ T, const float *__restrict__ Y,
+                                                  float *__restrict__ h_out, const ThermoDev *__restrict__ th) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double t = (double)T[i];
+    const int Ns = th->n_species, two = th->two_ranges;
+    double s = 0.0;
+    for (int k = 0; k < Ns; ++k) {
+        const int r = (two && !(t < th->T_mid[k])) ? 1 : 0;
+        const double *hh = th->hh[k][r];
+        const double hk = hh[0] + t * (hh[1] + t * (hh[2] + t * (hh[3] + t * (hh[4] + t * hh[5]))));
+        s = fma((double)Y[(int64_t)k * n + i], hk, s);
+    }
+    h_out[i] = (float)s;
+}
+
+cudaError_t launch_enthalpy(Ctx *c, int64_t n, const float *T, const float *Y, float *h_out, cudaStream_t s) {
+    if (n <= 0) return cudaSuccess;
+    k_enthalpy<<<(unsigned)((n + 127) / 128), 128, 0, s>>>(n, T, Y, h_out, c->thermo_dev);
+    c->launches += 1;
+    return cudaGetLastError();
+}
+
+// G4: per-feature sum of (x - shift)^power over the batch, FP64, x = {T, p, F(Y_k)} with the FP64 Box-Cox of
+// the FP32 Y.  Per-block partial sums; the host adds them in block order (deterministic).
+constexpr int kMomThreads = 256;
+__global__ void __launch_bounds__(kMomThreads) k_moment_partial(int64_t n, int D, const float *__restrict__ T,
+                                                                const float *__restrict__ p,
+                                                                const float *__restrict__ Y, double lambda,
+                                                                const double *__restrict__ shift, int square,
+                                                                double *__restrict__ partial /* [gridDim.x][D] */) {
+    __shared__ double red[kMomThreads / 32];
+    for (int j = 0; j < D; ++j) {
+        const double sh = shift ? shift[j] : 0.0;
+        double acc = 0.0;
+        for (int64_t i = (int64_t)blockIdx.x * kMomThreads + threadIdx.x; i < n; i += (int64_t)gridDim.x * kMomThreads) {
+            double x;
+            if (j == 0) x = (double)T[i];
+            else if (j == 1) x = (double)p[i];
+            else {
+                double yc = (double)Y[(int64_t)(j - 2) * n + i];
+                if (yc < 0.0) yc = 0.0;
+                x = lambda != 0.0 ? (pow(yc, lambda) - 1.0) / lambda : log(yc);
+            }
+            x -= sh;
+            acc += square ? x * x : x;
+        }
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, d);
+        if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = acc;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double t = 0.0;
+            for (int w = 0; w < kMomThreads / 32; ++w) t += red[w];
+            partial[(size_t)blockIdx.x * D + j] = t;
+        }
+        __syncthreads();
+    }
+}
+
+cudaError_t launch_moments(Ctx *c, int64_t n, int Ns, const float *T, const float *p, const float *Y, double lambda,
+                           double *mean_out, double *std_out, cudaStream_t s) {
+    const int D = Ns + 2;
+    const int blocks = 2 * (c->sm_count > 0 ? c->sm_count : 148);
+    double *partial = nullptr, *shift = nullptr;
+    cudaError_t e = cudaMalloc(&partial, sizeof(double) * (size_t)blocks * D);
+    if (e != cudaSuccess) return e;
+    e = cudaMalloc(&shift, sizeof(double) * D);
+    if (e != cudaSuccess) {
+        cudaFree(partial);
+        return e;
+    }
+    std::vector<double> hp((size_t)blocks * D), mean(D);
+    for (int pass = 0; pass < 2 && e == cudaSuccess; ++pass) {
+        k_moment_partial<<<blocks, kMomThreads, 0, s>>>(n, D, T, p, Y, lambda, pass ? shift : nullptr, pass, partial);
+        c->launches += 1;
+        e = cudaGetLastError();
+        if (e == cudaSuccess)
+            e = cudaMemcpyAsync(hp.data(), partial, sizeof(double) * hp.size(), cudaMemcpyDeviceToHost, s);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+        if (e != cudaSuccess) break;
+        for (int j = 0; j < D; ++j) {
+            double t = 0.0;
+            for (int b = 0; b < blocks; ++b) t += hp[(size_t)b * D + j];
+            if (pass == 0) {
+                mean[j] = t / (double)n;
+                mean_out[j] = mean[j];
+            } else {
+                std_out[j] = sqrt(t / (double)n);
+            }
+        }
+        if (pass == 0) e = cudaMemcpyAsync(shift, mean.data(), sizeof(double) * D, cudaMemcpyHostToDevice, s);
+    }
+    cudaStreamSynchronize(s);
+    cudaFree(partial);
+    cudaFree(shift);
+    return e;
+}
+
+}  // namespace gpuann

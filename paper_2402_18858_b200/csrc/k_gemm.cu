@@ -1,0 +1,285 @@
+// k_gemm.cu -- one fully connected layer of S3 on the 5th-generation tensor cores ("bf16-layerwise" variant):
+//     out[r][j] = act( sum_i A[r][i] W[j][i] + b[j] ),   A: [rows][Kp] BF16, W: [Np][Kp] BF16, FP32 accumulate
+// (PAPER.md:103 hidden sizes / GELU; PAPER.md:56 half-precision inference).  Persistent, warp-specialised:
+//   warp 0    TMA producer: A tile 128 x 64 and W tile n_tile x 64 (128-byte swizzle) into a 4-stage ring
+//   warp 1    allocates TMEM (512 columns = 2 accumulators of <= 256 columns) and issues tcgen05.mma
+//             (M = 128, N = n_tile, K = 16), committing each stage back to the producer and each finished
+//             accumulator to the epilogue
+//   warps 2-5 epilogue: tcgen05.ld 32 lanes x 16 columns, + bias, GELU, BF16 pack, 2 x 16-byte stores per row
+//             (hidden layers) or FP32 species-major stores (last layer); overlaps the next tile's MMAs.
+// Tiles are walked n-fastest so that CTAs running together share the A rows and the whole W in L2.
+#include "common.cuh"
+#include "ptx.cuh"
+
+namespace gpuann {
+
+constexpr int kBM = 128;
+constexpr int kBK = 64;
+constexpr int kStages = 4;
+constexpr int kMaxNT = 256;
+constexpr int kGemmThreads = 192;
+constexpr uint32_t kABytes = kBM * kBK * 2;        // 16 KB
+constexpr uint32_t kBBytesMax = kMaxNT * kBK * 2;  // 32 KB
+constexpr size_t kGemmSmem = 1024 /*align slack*/ + (size_t)kStages * (kABytes + kBBytesMax) + 256;
+
+// GELU in the tanh form, tanh.approx.f32 (R5: any evaluation inside the BF16 tolerances)
+__device__ __forceinline__ float gelu_tanh(float v) {
+    const float u = v * (0.7978845608028654f + 0.0356774081363001f * v * v);
+    const float hv = 0.5f * v;
+    return fmaf(hv, ptx::tanh_approx(u), hv);
+}
+
+struct GemmArgs {
+    int Kp, Np, N;          // padded K, padded N, true N
+    int n_tile, tiles_n;
+    int64_t rows;           // valid rows when n_active == nullptr
+    int64_t c0;             // first (compacted) cell of this chunk, for the n_active test
+    const int32_t *n_active;  // DEVICE or nullptr: rows = clamp(*n_active - c0, 0, rows)
+    const float *bias;      // [Np]
+    __nv_bfloat16 *out_bf16;  // [rows][out_ld] or nullptr
+    int out_ld;
+    float *out_f32;         // [N][out_f32_stride] (species-major) or nullptr
+    int64_t out_f32_stride;
+    int apply_gelu;
+};
+
+__global__ void __launch_bounds__(kGemmThreads, 1)
+k_layer_bf16(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ CUtensorMap tmapW, const GemmArgs ga) {
+    extern __shared__ unsigned char smem_raw[];
+    unsigned char *smem = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    unsigned char *sA = smem;
+    unsigned char *sB = smem + (size_t)kStages * kABytes;
+    uint64_t *bars = reinterpret_cast<uint64_t *>(sB + (size_t)kStages * kBBytesMax);
+    uint64_t *full = bars, *empty = bars + kStages, *tfull = bars + 2 * kStages, *tempty = bars + 2 * kStages + 2;
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(bars + 2 * kStages + 4);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    int64_t rows = ga.rows;
+    if (ga.n_active) {
+        int64_t r = (int64_t)*ga.n_active - ga.c0;
+        rows = r < 0 ? 0 : (r < rows ? r : rows);
+    }
+    const int tiles_m = (int)((rows + kBM - 1) / kBM);
+    const int n_tiles = tiles_m * ga.tiles_n;
+    const int num_kb = (ga.Kp + kBK - 1) / kBK;
+    const uint32_t b_bytes = (uint32_t)ga.n_tile * kBK * 2;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < kStages; ++s) {
+            ptx::mbar_init(&full[s], 1);
+            ptx::mbar_init(&empty[s], 1);
+        }
+        for (int a = 0; a < 2; ++a) {
+            ptx::mbar_init(&tfull[a], 1);
+            ptx::mbar_init(&tempty[a], 4);
+        }
+        ptx::fence_mbar_init();
+    }
+    if (warp == 0 && lane == 0) {
+        ptx::prefetch_tensormap(&tmapA);
+        ptx::prefetch_tensormap(&tmapW);
+    }
+    if (warp == 1) {
+        ptx::tmem_alloc(tmem_slot, 512);
+        ptx::tmem_relinquish();
+    }
+    ptx::tc_fence_before_sync();
+    __syncthreads();
+    ptx::tc_fence_after_sync();
+    const uint32_t tmem_base = *tmem_slot;
+
+    if (warp == 0) {
+        // ===================================================== TMA producer
+        if (lane == 0) {
+            int stage = 0;
+            uint32_t phase = 0;
+            for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+                const int mt = tile / ga.tiles_n, nt = tile % ga.tiles_n;
+                for (int kb = 0; kb < num_kb; ++kb) {
+                    ptx::mbar_wait(&empty[stage], phase ^ 1);
+                    ptx::mbar_arrive_expect_tx(&full[stage], kABytes + b_bytes);
+                    ptx::tma_load_2d(&tmapA, &full[stage], sA + (size_t)stage * kABytes, kb * kBK, mt * kBM);
+                    ptx::tma_load_2d(&tmapW, &full[stage], sB + (size_t)stage * kBBytesMax, kb * kBK, nt * ga.n_tile);
+                    if (++stage == kStages) {
+                        stage = 0;
+                        phase ^= 1;
+                    }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===================================================== MMA issuer
+        if (lane == 0) {
+            int stage = 0;
+            uint32_t phase = 0;
+            int it = 0;
+            for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+                const int nt = tile % ga.tiles_n;
+                const int n_cur = min(ga.n_tile, ga.Np - nt * ga.n_tile);
+                const uint32_t idesc = ptx::umma_idesc_bf16_f32(kBM, (uint32_t)n_cur);
+                const int acc = it & 1;
+                const uint32_t acc_phase = (uint32_t)(it >> 1) & 1;
+                ptx::mbar_wait(&tempty[acc], acc_phase ^ 1);
+                ptx::tc_fence_after_sync();
+                const uint32_t d_tmem = tmem_base + (uint32_t)acc * kMaxNT;
+                for (int kb = 0; kb < num_kb; ++kb) {
+                    ptx::mbar_wait(&full[stage], phase);
+                    ptx::tc_fence_after_sync();
+                    const uint32_t a_addr = ptx::smem_u32(sA + (size_t)stage * kABytes);
+                    const uint32_t b_addr = ptx::smem_u32(sB + (size_t)stage * kBBytesMax);
+                    const int ksteps = min(kBK / 16, (ga.Kp - kb * kBK) / 16);
+                    for (int k = 0; k < ksteps; ++k) {
+                        const uint64_t da = ptx::umma_desc_sw128_kmajor(a_addr + k * 32);
+                        const uint64_t db = ptx::umma_desc_sw128_kmajor(b_addr + k * 32);
+                        ptx::umma_bf16_ss(d_tmem, da, db, idesc, (kb | k) ? 1u : 0u);
+                    }
+                    ptx::umma_commit(&empty[stage]);  // frees the smem slot when these MMAs have read it
+                    if (++stage == kStages) {
+                        stage = 0;
+                        phase ^= 1;
+                    }
+                }
+                ptx::umma_commit(&tfull[acc]);  // accumulator complete -> epilogue
+            }
+        }
+    } else {
+        // ===================================================== epilogue (warps 2..5)
+        const int q = warp & 3;  // TMEM lane quarter this warp may access
+        int it = 0;
+        for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+            const int mt = tile / ga.tiles_n, nt = tile % ga.tiles_n;
+            const int n_cur = min(ga.n_tile, ga.Np - nt * ga.n_tile);
+            const int acc = it & 1;
+            const uint32_t acc_phase = (uint32_t)(it >> 1) & 1;
+            ptx::mbar_wait(&tfull[acc], acc_phase);
+            ptx::tc_fence_after_sync();
+            const int64_t r = (int64_t)mt * kBM + q * 32 + lane;
+            const bool row_ok = r < rows;
+            const uint32_t t_addr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)acc * kMaxNT;
+            const int col0 = nt * ga.n_tile;
+            for (int cc = 0; cc < n_cur; cc += 16) {
+                uint32_t v[16];
+                ptx::tmem_ld16(t_addr + cc, v);
+                ptx::tmem_ld_wait();
+                float f[16];
+                const float4 *b4 = reinterpret_cast<const float4 *>(ga.bias + col0 + cc);
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const float4 b = __ldg(b4 + j);
+                    f[4 * j + 0] = __uint_as_float(v[4 * j + 0]) + b.x;
+                    f[4 * j + 1] = __uint_as_float(v[4 * j + 1]) + b.y;
+                    f[4 * j + 2] = __uint_as_float(v[4 * j + 2]) + b.z;
+                    f[4 * j + 3] = __uint_as_float(v[4 * j + 3]) + b.w;
+                }
+                if (ga.apply_gelu) {
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) f[j] = gelu_tanh(f[j]);
+                }
+                if (ga.out_bf16) {
+                    if (row_ok) {
+                        uint4 o0, o1;
+                        o0.x = ptx::pack_bf16x2(f[0], f[1]);
+                        o0.y = ptx::pack_bf16x2(f[2], f[3]);
+                        o0.z = ptx::pack_bf16x2(f[4], f[5]);
+                        o0.w = ptx::pack_bf16x2(f[6], f[7]);
+                        o1.x = ptx::pack_bf16x2(f[8], f[9]);
+                        o1.y = ptx::pack_bf16x2(f[10], f[11]);
+                        o1.z = ptx::pack_bf16x2(f[12], f[13]);
+                        o1.w = ptx::pack_bf16x2(f[14], f[15]);
+                        uint4 *dst = reinterpret_cast<uint4 *>(ga.out_bf16 + r * ga.out_ld + col0 + cc);
+                        dst[0] = o0;
+                        dst[1] = o1;
+                    }
+                } else if (row_ok) {
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) {
+                        const int col = col0 + cc + j;
+                        if (col < ga.N) ga.out_f32[(int64_t)col * ga.out_f32_stride + r] = f[j];
+                    }
+                }
+            }
+            ptx::tc_fence_before_sync();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(&tempty[acc]);
+        }
+    }
+
+    ptx::tc_fence_before_sync();
+    __syncthreads();
+    if (warp == 1) {
+        ptx::tc_fence_after_sync();
+        ptx::tmem_dealloc(tmem_base, 512);
+    }
+}
+
+// ---------------------------------------------------------------- host side
+typedef CUresult (*PFN_encodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                    const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static PFN_encodeTiled get_encode_fn(std::string *err) {
+    static PFN_encodeTiled fn = nullptr;
+    if (fn) return fn;
+    void *p = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres);
+    if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !p) {
+        if (err) *err = std::string("cuTensorMapEncodeTiled is not available: ") + cudaGetErrorString(e);
+        return nullptr;
+    }
+    fn = reinterpret_cast<PFN_encodeTiled>(p);
+    return fn;
+}
+
+bool encode_tmap_bf16(CUtensorMap *out, const void *base, uint64_t cols, uint64_t rows, uint64_t row_pitch_bytes,
+                      uint32_t box_rows, std::string *err) {
+    PFN_encodeTiled fn = get_encode_fn(err);
+    if (!fn) return false;
+    cuuint64_t dims[2] = {cols, rows};
+    cuuint64_t strides[1] = {row_pitch_bytes};
+    cuuint32_t box[2] = {(cuuint32_t)kBK, box_rows};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = fn(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void *>(base), dims, strides, box, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        if (err) *err = "cuTensorMapEncodeTiled failed with CUresult " + std::to_string((int)r);
+        return false;
+    }
+    return true;
+}
+
+cudaError_t gemm_setup(Ctx *c) {
+    (void)c;
+    return cudaFuncSetAttribute(k_layer_bf16, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kGemmSmem);
+}
+
+cudaError_t launch_layer_bf16(Ctx *c, int layer, int64_t rows, const CUtensorMap *tmapA, __nv_bfloat16 *out_bf16,
+                              int out_ld, float *out_f32, int64_t out_f32_stride, int64_t c0, bool use_count,
+                              cudaStream_t s) {
+    if (rows <= 0) return cudaSuccess;
+    const LayerBf16 &ly = c->lay[layer];
+    GemmArgs ga{};
+    ga.Kp = ly.Kp;
+    ga.Np = ly.Np;
+    ga.N = ly.N;
+    ga.n_tile = ly.n_tile;
+    ga.tiles_n = ly.tiles_n;
+    ga.rows = rows;
+    ga.c0 = c0;
+    ga.n_active = use_count ? c->n_active_dev : nullptr;
+    ga.bias = ly.bias;
+    ga.out_bf16 = out_bf16;
+    ga.out_ld = out_ld;
+    ga.out_f32 = out_f32;
+    ga.out_f32_stride = out_f32_stride;
+    ga.apply_gelu = (layer < c->L - 1) ? 1 : 0;
+    const int64_t tiles = ((rows + kBM - 1) / kBM) * ly.tiles_n;
+    const int grid = (int)(tiles < c->sm_count ? tiles : c->sm_count);
+    k_layer_bf16<<<grid, kGemmThreads, kGemmSmem, s>>>(*tmapA, ly.tmapW, ga);
+    c->launches += 1;
+    return cudaGetLastError();
+}
+
+}  // namespace gpuann

@@ -1,0 +1,163 @@
+"""Shared plumbing of the `-m gpu` parity tests: build the seeded problem, derive (h, normalisation) with the
+oracle, run the CUDA path through the C ABI (ctypes binding) and the oracle on the same FP32 inputs.
+
+Tolerances (BASELINE.json north_star):
+  FP32 path: |Y - Y_ref| <= 1e-5 |Y_ref| + 1e-10, max |T - T_ref| <= 1e-3 K
+  BF16 path: per output column ||o - o_ref||_2 <= 2e-2 ||o_ref||_2 and max|o - o_ref| <= 2e-2 max|o_ref|,
+             max |T - T_ref| <= 0.5 K
+  both:      max |sum_k Y_new - 1| <= 1e-6 (FP64 sum of the stored FP32 values)
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass
+from typing import Optional
+
+import numpy as np
+
+import oracle
+from paper_2402_18858_b200 import binding as B
+from paper_2402_18858_b200 import inputs as I
+
+
+@dataclass
+class Prepared:
+    prob: I.Problem
+    h: np.ndarray        # [n] f32
+    in_mean: np.ndarray  # [2+Ns] f32
+    in_std: np.ndarray
+    model: oracle.OracleModel
+
+
+def prepare(cfg: I.Config, n: Optional[int] = None, seed: Optional[int] = None, **over) -> Prepared:
+    # tiny batches take their normalisation statistics from a 4,096-cell batch of the same seed, then keep n cells
+    n_gen = None if n is None else max(int(n), 4096)
+    prob = I.make_problem(cfg, n=n_gen, seed=seed)
+    st, th = prob.state, prob.thermo
+    mean, std = oracle.input_moments(st.T, st.p, st.Y, cfg.lam)                                       # G4
+    if n is not None and n_gen != n:
+        st = I.State(st.T[:n].copy(), st.p[:n].copy(), np.ascontiguousarray(st.Y[:, :n]))
+        prob = I.Problem(prob.cfg, int(n), st, th, prob.net, prob.out_mean, prob.out_std)
+    h = oracle.enthalpy_field(st.T, st.Y, th.nasa_lo, th.nasa_hi, th.T_mid, th.W).astype(np.float32)  # G5
+    in_mean, in_std = mean.astype(np.float32), std.astype(np.float32)
+    model = oracle.OracleModel(
+        sizes=prob.net.sizes, weights=prob.net.weights, biases=prob.net.biases, in_mean=in_mean, in_std=in_std,
+        out_mean=prob.out_mean, out_std=prob.out_std, lam=cfg.lam, nasa_lo=th.nasa_lo, W=th.W, nasa_hi=th.nasa_hi,
+        T_mid=th.T_mid, T_min=cfg.T_min, T_max=cfg.T_max, newton_tol=cfg.newton_tol,
+        newton_max_iter=over.get("newton_max_iter", cfg.newton_max_iter), T_active=over.get("T_active", cfg.T_active))
+    return Prepared(prob, h, in_mean, in_std, model)
+
+
+def make_ctx(pr: Prepared, precision: Optional[int] = None, chunk_cells: int = 0) -> int:
+    cfg = pr.prob.cfg
+    prm = B.gpuann_default_params()
+    prm.precision = cfg.precision if precision is None else precision
+    prm.newton_max_iter = pr.model.newton_max_iter
+    prm.newton_tol = pr.model.newton_tol
+    prm.T_min, prm.T_max = pr.model.T_min, pr.model.T_max
+    prm.T_active = pr.model.T_active
+    prm.chunk_cells = chunk_cells
+    ctx = B.gpuann_create(prm)
+    try:
+        B.gpuann_load_net(ctx, cfg.n_species, pr.prob.net.sizes, pr.prob.net.weights, pr.prob.net.biases,
+                          pr.in_mean, pr.in_std, pr.prob.out_mean, pr.prob.out_std, cfg.lam)
+        th = pr.prob.thermo
+        B.gpuann_load_thermo(ctx, cfg.n_species, th.nasa_lo, th.nasa_hi, th.T_mid, th.W)
+    except Exception:
+        B.gpuann_destroy(ctx)
+        raise
+    return ctx
+
+
+@dataclass
+class GpuResult:
+    T_new: np.ndarray   # [n] f32
+    Y_new: np.ndarray   # [Ns][n] f32
+    o_raw: Optional[np.ndarray]
+    stats: tuple
+
+
+def run_gpu(ctx: int, pr: Prepared, T=None, p=None, Y=None, h=None, want_raw: bool = True, dt: Optional[float] = None,
+            use_stream: bool = True) -> GpuResult:
+    import torch
+    st = pr.prob.state
+    T = st.T if T is None else T
+    p = st.p if p is None else p
+    Y = st.Y if Y is None else Y
+    h = pr.h if h is None else h
+    n = int(T.shape[0])
+    Ns = pr.prob.cfg.n_species
+    dev = torch.device("cuda:0")
+    dT = torch.from_numpy(np.ascontiguousarray(T)).to(dev)
+    dp = torch.from_numpy(np.ascontiguousarray(p)).to(dev)
+    dY = torch.from_numpy(np.ascontiguousarray(Y)).to(dev)
+    dh = torch.from_numpy(np.ascontiguousarray(h)).to(dev)
+    stream = torch.cuda.current_stream().cuda_stream if use_stream else 0
+    o_raw = None
+    if want_raw:
+        dO = torch.full((Ns, max(n, 1)), float("nan"), dtype=torch.float32, device=dev)
+        B.gpuann_debug_forward(ctx, n, dT.data_ptr(), dp.data_ptr(), dY.data_ptr(), dO.data_ptr(), stream)
+        torch.cuda.synchronize()
+        o_raw = dO.cpu().numpy()[:, :n]
+    B.gpuann_reset_stats(ctx)
+    B.gpuann_chem_step(ctx, n, dT.data_ptr(), dp.data_ptr(), dY.data_ptr(), dh.data_ptr(),
+                       pr.prob.cfg.dt if dt is None else dt, stream)
+    torch.cuda.synchronize()
+    stats = B.gpuann_get_stats(ctx)
+    return GpuResult(dT.cpu().numpy(), dY.cpu().numpy(), o_raw, stats)
+
+
+def run_oracle(pr: Prepared, T=None, p=None, Y=None, h=None, dt: Optional[float] = None):
+    st = pr.prob.state
+    o = oracle.Oracle(pr.model)
+    return o.chem_step(st.T if T is None else T, st.p if p is None else p, st.Y if Y is None else Y,
+                       pr.h if h is None else h, pr.prob.cfg.dt if dt is None else dt)
+
+
+def run_oracle_all_active(pr: Prepared):
+    """The oracle with the active-cell test off (gpuann_debug_forward computes every cell, skipped or not)."""
+    import dataclasses
+    m = dataclasses.replace(pr.model, T_active=0.0)
+    st = pr.prob.state
+    return oracle.Oracle(m).chem_step(st.T, st.p, st.Y, pr.h, pr.prob.cfg.dt)
+
+
+# ------------------------------------------------------------------ the comparisons
+def check_sumY(Y_new: np.ndarray, mask=None):
+    s = Y_new.astype(np.float64).sum(axis=0)
+    if mask is not None:
+        s = s[mask]
+    dev = np.abs(s - 1.0).max() if s.size else 0.0
+    assert dev <= 1e-6, f"max |sum Y - 1| = {dev:.3e} > 1e-6"
+    return dev
+
+
+def check_fp32(g: GpuResult, ref, mask=None):
+    sel = slice(None) if mask is None else mask
+    Yg, Yr = g.Y_new.astype(np.float64)[:, sel], ref.Y_new[:, sel]
+    err = np.abs(Yg - Yr)
+    tol = 1e-5 * np.abs(Yr) + 1e-10
+    worst = (err / tol).max() if err.size else 0.0
+    assert worst <= 1.0, f"Y_new: max err/tol = {worst:.3f} (tol = 1e-5 |Y| + 1e-10)"
+    dT = np.abs(g.T_new.astype(np.float64)[sel] - ref.T_new[sel])
+    assert (dT.max() if dT.size else 0.0) <= 1e-3, f"T_new: max |dT| = {dT.max():.3e} K > 1e-3 K"
+    return worst, (dT.max() if dT.size else 0.0)
+
+
+def check_raw_bf16(o_gpu: np.ndarray, o_ref: np.ndarray, mask=None):
+    sel = slice(None) if mask is None else mask
+    og, orf = o_gpu.astype(np.float64)[:, sel], o_ref[:, sel]
+    assert np.isfinite(og).all(), "raw output has non-finite entries"
+    d = og - orf
+    l2 = np.sqrt((d * d).sum(axis=1)) / np.sqrt((orf * orf).sum(axis=1))
+    mx = np.abs(d).max(axis=1) / np.abs(orf).max(axis=1)
+    assert l2.max() <= 2e-2, f"raw output: column rel-L2 {l2.max():.3e} > 2e-2"
+    assert mx.max() <= 2e-2, f"raw output: column max|d|/max|ref| {mx.max():.3e} > 2e-2"
+    return l2.max(), mx.max()
+
+
+def check_T_bf16(g: GpuResult, ref, mask=None):
+    sel = slice(None) if mask is None else mask
+    dT = np.abs(g.T_new.astype(np.float64)[sel] - ref.T_new[sel])
+    m = dT.max() if dT.size else 0.0
+    assert m <= 0.5, f"T_new: max |dT| = {m:.3e} K > 0.5 K"
+    return m

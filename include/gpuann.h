@@ -160,6 +160,17 @@ int gpuann_input_moments(gpuann_ctx *ctx, int64_t n_cells, int n_species, const 
 /* Number of kernel launches this context has enqueued so far (bench.py reports it as gpu_launches). */
 int64_t gpuann_launch_count(const gpuann_ctx *ctx);
 
+/* Per-kernel device timing, for the roofline arithmetic of bench.py.  While enabled, every kernel launch of
+ * this context is bracketed by two CUDA events on the launching stream (a small host cost per launch, so the
+ * headline throughput is measured with timing off).  gpuann_timing_read synchronises the last stream, writes
+ * for each kernel class i < n_classes the summed device time ms[i] and the number of launches counts[i]
+ * recorded since the last enable/read, and clears the record.  Classes: gpuann_timing_num_classes() of them,
+ * named by gpuann_timing_class_name ("layer1_gemm", "post_update_newton", ...; "" if out of range). */
+int gpuann_timing_enable(gpuann_ctx *ctx, int enable);
+int gpuann_timing_read(gpuann_ctx *ctx, int n_classes, double *ms, int64_t *counts);
+int gpuann_timing_num_classes(void);
+const char *gpuann_timing_class_name(int cls);
+
 /* Static description of the work one chem_step does, for roofline arithmetic: MACs the tensor path
  * issues per cell including K/N padding (0 on the FP32 path), and the name of the kernel variant chosen
  * for the loaded net ("fp32", "bf16-layerwise", "bf16-fused").  Any out pointer may be NULL. */

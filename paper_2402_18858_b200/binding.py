@@ -27,7 +27,8 @@ GPUANN_PRECISION_BF16 = 1
 SYMBOLS = [
     "gpuann_default_params", "gpuann_create", "gpuann_load_net", "gpuann_load_thermo", "gpuann_chem_step",
     "gpuann_chem_step_host", "gpuann_debug_forward", "gpuann_get_stats", "gpuann_reset_stats", "gpuann_enthalpy",
-    "gpuann_input_moments", "gpuann_launch_count", "gpuann_describe", "gpuann_last_error", "gpuann_destroy",
+    "gpuann_input_moments", "gpuann_launch_count", "gpuann_timing_enable", "gpuann_timing_read",
+    "gpuann_timing_num_classes", "gpuann_timing_class_name", "gpuann_describe", "gpuann_last_error", "gpuann_destroy",
 ]
 
 
@@ -84,6 +85,14 @@ def lib() -> C.CDLL:
     L.gpuann_input_moments.argtypes = [vp, i64, C.c_int, vp, vp, vp, dbl, vp, vp, vp]
     L.gpuann_launch_count.restype = i64
     L.gpuann_launch_count.argtypes = [vp]
+    L.gpuann_timing_enable.restype = C.c_int
+    L.gpuann_timing_enable.argtypes = [vp, C.c_int]
+    L.gpuann_timing_read.restype = C.c_int
+    L.gpuann_timing_read.argtypes = [vp, C.c_int, C.POINTER(dbl), C.POINTER(i64)]
+    L.gpuann_timing_num_classes.restype = C.c_int
+    L.gpuann_timing_num_classes.argtypes = []
+    L.gpuann_timing_class_name.restype = C.c_char_p
+    L.gpuann_timing_class_name.argtypes = [C.c_int]
     L.gpuann_describe.restype = C.c_int
     L.gpuann_describe.argtypes = [vp, C.POINTER(i64), C.POINTER(C.c_char_p)]
     L.gpuann_last_error.restype = C.c_char_p
@@ -197,6 +206,19 @@ def gpuann_input_moments(ctx: int, n_cells: int, n_species: int, T: int, p: int,
 
 def gpuann_launch_count(ctx: int) -> int:
     return int(lib().gpuann_launch_count(ctx))
+
+
+def gpuann_timing_enable(ctx: int, enable: bool) -> None:
+    _check(lib().gpuann_timing_enable(ctx, 1 if enable else 0), ctx)
+
+
+def gpuann_timing_read(ctx: int) -> dict:
+    """Returns {class name: (summed device ms, launches)} for the classes that launched since the last enable/read."""
+    n = lib().gpuann_timing_num_classes()
+    ms = (C.c_double * n)()
+    cnt = (C.c_int64 * n)()
+    _check(lib().gpuann_timing_read(ctx, n, ms, cnt), ctx)
+    return {lib().gpuann_timing_class_name(i).decode(): (ms[i], cnt[i]) for i in range(n) if cnt[i] > 0}
 
 
 def gpuann_describe(ctx: int):

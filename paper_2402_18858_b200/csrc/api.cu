@@ -530,6 +530,56 @@ int gpuann_input_moments(gpuann_ctx *c, int64_t n, int n_species, const float *T
 
 int64_t gpuann_launch_count(const gpuann_ctx *c) { return c ? c->launches : 0; }
 
+static void recycle_timed(Ctx *c) {
+    for (auto &t : c->timed) {
+        c->event_pool.push_back(t.e0);
+        c->event_pool.push_back(t.e1);
+    }
+    c->timed.clear();
+}
+
+int gpuann_timing_enable(gpuann_ctx *c, int enable) {
+    if (!c) return fail(nullptr, GPUANN_ERR_INVALID_ARG, "gpuann_timing_enable: ctx is NULL");
+    DeviceGuard g(c->device);
+    CU_TRY(c, cudaStreamSynchronize(c->last_stream), "cudaStreamSynchronize");
+    recycle_timed(c);
+    c->timing = enable != 0;
+    return GPUANN_OK;
+}
+
+int gpuann_timing_read(gpuann_ctx *c, int n_classes, double *ms, int64_t *counts) {
+    if (!c) return fail(nullptr, GPUANN_ERR_INVALID_ARG, "gpuann_timing_read: ctx is NULL");
+    if (n_classes < 0 || (n_classes > 0 && (!ms || !counts)))
+        return fail(c, GPUANN_ERR_INVALID_ARG, "gpuann_timing_read: bad argument");
+    DeviceGuard g(c->device);
+    CU_TRY(c, cudaStreamSynchronize(c->last_stream), "cudaStreamSynchronize");
+    for (int i = 0; i < n_classes; ++i) {
+        ms[i] = 0.0;
+        counts[i] = 0;
+    }
+    for (auto &t : c->timed) {
+        float dtm = 0.f;
+        cudaError_t e = cudaEventElapsedTime(&dtm, t.e0, t.e1);
+        if (e != cudaSuccess) return fail_cuda(c, e, "cudaEventElapsedTime");
+        if (t.cls >= 0 && t.cls < n_classes) {
+            ms[t.cls] += (double)dtm;
+            counts[t.cls] += 1;
+        }
+    }
+    recycle_timed(c);
+    return GPUANN_OK;
+}
+
+int gpuann_timing_num_classes(void) { return kNumKernelClasses; }
+
+const char *gpuann_timing_class_name(int cls) {
+    static const char *names[kNumKernelClasses] = {"compact",      "pre_boxcox_norm", "layer0_gemm", "layer1_gemm",
+                                                   "layer2_gemm",  "layer3_gemm",     "layer4_gemm", "layer5_gemm",
+                                                   "layer6_gemm",  "layer7_gemm",     "post_update_newton",
+                                                   "fp32_fused",   "bf16_fused",      "aux"};
+    return (cls >= 0 && cls < kNumKernelClasses) ? names[cls] : "";
+}
+
 int gpuann_describe(const gpuann_ctx *c, int64_t *issued_mac_per_cell, const char **variant) {
     if (!c) return GPUANN_ERR_INVALID_ARG;
     if (issued_mac_per_cell) *issued_mac_per_cell = c->issued_mac_per_cell;
@@ -551,6 +601,9 @@ int gpuann_destroy(gpuann_ctx *c) {
         cudaFree(c->n_active_dev);
         cudaFree(c->stage);
         cudaFree(c->counters);
+        recycle_timed(c);
+        for (cudaEvent_t e : c->event_pool) cudaEventDestroy(e);
+        c->event_pool.clear();
         if (c->own_stream) cudaStreamDestroy(c->own_stream);
         cudaGetLastError();
     }

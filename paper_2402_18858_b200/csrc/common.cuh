@@ -120,6 +120,54 @@ struct Ctx {
     cudaStream_t own_stream = nullptr;  // used by gpuann_chem_step_host
     cudaStream_t last_stream = nullptr;
     int64_t launches = 0;
+
+    // per-kernel-class device timing (gpuann_timing_enable / gpuann_timing_read): CUDA events around every launch
+    bool timing = false;
+    struct TimedLaunch {
+        int cls;
+        cudaEvent_t e0, e1;
+    };
+    std::vector<TimedLaunch> timed;       // launches recorded since timing was enabled
+    std::vector<cudaEvent_t> event_pool;  // recycled events
+};
+
+// Kernel classes of the timing hook (index into gpuann_timing_read's arrays)
+enum KernelClass {
+    kClsCompact = 0,
+    kClsPre = 1,
+    kClsLayer0 = 2,  // + layer index (0..7)
+    kClsPost = 10,
+    kClsFp32 = 11,
+    kClsFused = 12,
+    kClsAux = 13,
+    kNumKernelClasses = 14
+};
+
+// RAII: counts the launch and, when timing is on, brackets it with two events on the launching stream.
+struct LaunchScope {
+    Ctx *c;
+    cudaStream_t s;
+    cudaEvent_t e1 = nullptr;
+    LaunchScope(Ctx *ctx, int cls, cudaStream_t stream, int n_launches = 1) : c(ctx), s(stream) {
+        c->launches += n_launches;
+        if (!c->timing) return;
+        cudaEvent_t ev[2] = {nullptr, nullptr};
+        for (int i = 0; i < 2; ++i) {
+            if (!c->event_pool.empty()) {
+                ev[i] = c->event_pool.back();
+                c->event_pool.pop_back();
+            } else if (cudaEventCreate(&ev[i]) != cudaSuccess) {
+                ev[i] = nullptr;
+            }
+        }
+        if (!ev[0] || !ev[1]) return;
+        cudaEventRecord(ev[0], s);
+        e1 = ev[1];
+        c->timed.push_back({cls, ev[0], ev[1]});
+    }
+    ~LaunchScope() {
+        if (e1) cudaEventRecord(e1, s);
+    }
 };
 
 // ---------------------------------------------------------------- kernel launchers (defined in the .cu files)

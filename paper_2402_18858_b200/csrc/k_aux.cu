@@ -97,10 +97,10 @@ __global__ void __launch_bounds__(kCompThreads) k_compact_scatter(int64_t n, con
 
 cudaError_t launch_compact(Ctx *c, int64_t n, const float *T, float T_active, cudaStream_t s) {
     const int nb = (int)((n + kCompPerBlock - 1) / kCompPerBlock);
+    LaunchScope ls(c, kClsCompact, s, 3);
     k_compact_count<<<nb, kCompThreads, 0, s>>>(n, T, T_active, c->blk_counts);
     k_compact_scan<<<1, kCompThreads, 0, s>>>(nb, c->blk_counts, c->n_active_dev, c->counters);
     k_compact_scatter<<<nb, kCompThreads, 0, s>>>(n, T, T_active, c->blk_counts, c->idx);
-    c->launches += 3;
     return cudaGetLastError();
 }
 
@@ -155,8 +155,8 @@ cudaError_t launch_pre_bf16(Ctx *c, int64_t n, int64_t c0, int64_t cn, const flo
                             bool use_idx, __nv_bfloat16 *z, int Kp, cudaStream_t s) {
     if (cn <= 0) return cudaSuccess;
     const int blocks = (int)((cn + 127) / 128);
+    LaunchScope ls(c, kClsPre, s);
     k_pre_bf16<<<blocks, 128, 0, s>>>(n, c0, cn, T, p, Y, use_idx ? c->idx : nullptr, c->n_active_dev, z, Kp, c->pre);
-    c->launches += 1;
     return cudaGetLastError();
 }
 
@@ -217,10 +217,10 @@ cudaError_t launch_post(Ctx *c, int64_t n, int64_t c0, int64_t cn, float *T, flo
                         int64_t o_stride, double dt, bool use_idx, cudaStream_t s) {
     if (cn <= 0) return cudaSuccess;
     const int blocks = (int)((cn + 127) / 128);
+    LaunchScope ls(c, kClsPost, s);
     k_post<<<blocks, 128, sizeof(ThermoDev), s>>>(n, c0, cn, T, Y, h, o, o_stride, dt, use_idx ? c->idx : nullptr,
                                                    c->n_active_dev, c->thermo_dev, c->counters, (float)c->lambda,
                                                    c->post);
-    c->launches += 1;
     return cudaGetLastError();
 }
 
@@ -244,8 +244,8 @@ __global__ void __launch_bounds__(128) k_enthalpy(int64_t n, const float *__rest
 
 cudaError_t launch_enthalpy(Ctx *c, int64_t n, const float *T, const float *Y, float *h_out, cudaStream_t s) {
     if (n <= 0) return cudaSuccess;
+    LaunchScope ls(c, kClsAux, s);
     k_enthalpy<<<(unsigned)((n + 127) / 128), 128, 0, s>>>(n, T, Y, h_out, c->thermo_dev);
-    c->launches += 1;
     return cudaGetLastError();
 }
 
@@ -300,8 +300,10 @@ cudaError_t launch_moments(Ctx *c, int64_t n, int Ns, const float *T, const floa
     }
     std::vector<double> hp((size_t)blocks * D), mean(D);
     for (int pass = 0; pass < 2 && e == cudaSuccess; ++pass) {
-        k_moment_partial<<<blocks, kMomThreads, 0, s>>>(n, D, T, p, Y, lambda, pass ? shift : nullptr, pass, partial);
-        c->launches += 1;
+        {
+            LaunchScope ls(c, kClsAux, s);
+            k_moment_partial<<<blocks, kMomThreads, 0, s>>>(n, D, T, p, Y, lambda, pass ? shift : nullptr, pass, partial);
+        }
         e = cudaGetLastError();
         if (e == cudaSuccess)
             e = cudaMemcpyAsync(hp.data(), partial, sizeof(double) * hp.size(), cudaMemcpyDeviceToHost, s);

@@ -183,6 +183,7 @@ cudaError_t launch_chem_fp32(Ctx *c, int64_t n, float *T, const float *p, float 
     const unsigned blocks = (unsigned)((n + cb - 1) / cb);
     const float Tact = (float)c->prm.T_active;
     cudaError_t e = cudaSuccess;
+    LaunchScope ls(c, kClsFp32, s);
 #define GPUANN_LAUNCH_FP32(CB)                                                                                       \
     do {                                                                                                             \
         e = cudaFuncSetAttribute(k_chem_fp32<CB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);           \
@@ -196,7 +197,6 @@ cudaError_t launch_chem_fp32(Ctx *c, int64_t n, float *T, const float *p, float 
     else GPUANN_LAUNCH_FP32(8);
 #undef GPUANN_LAUNCH_FP32
     if (e != cudaSuccess) return e;
-    c->launches += 1;
     return cudaGetLastError();
 }
 

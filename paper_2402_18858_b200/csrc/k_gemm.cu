@@ -277,8 +277,8 @@ cudaError_t launch_layer_bf16(Ctx *c, int layer, int64_t rows, const CUtensorMap
     ga.apply_gelu = (layer < c->L - 1) ? 1 : 0;
     const int64_t tiles = ((rows + kBM - 1) / kBM) * ly.tiles_n;
     const int grid = (int)(tiles < c->sm_count ? tiles : c->sm_count);
+    LaunchScope ls(c, kClsLayer0 + layer, s);
     k_layer_bf16<<<grid, kGemmThreads, kGemmSmem, s>>>(*tmapA, ly.tmapW, ga);
-    c->launches += 1;
     return cudaGetLastError();
 }
 

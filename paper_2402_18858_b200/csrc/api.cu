@@ -1,6 +1,7 @@
 // api.cu -- the C ABI of libgpuann.so (include/gpuann.h): argument validation, context, weight / thermo
 // packing, the chunk loop of the tensor path.  Every step of the hot path runs in the kernels of k_*.cu.
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -66,6 +67,8 @@ void free_net(Ctx *c) {
         cudaFree(c->lay[l].bias);
         c->lay[l] = LayerBf16{};
     }
+    cudaFree(c->fused.W1p);
+    c->fused = FusedNet{};
     cudaFree(c->act[0]);
     cudaFree(c->act[1]);
     cudaFree(c->o_buf);
@@ -142,6 +145,7 @@ int gpuann_create(const gpuann_params *params, gpuann_ctx **out) {
     if (e == cudaSuccess) e = cudaMalloc(&c->thermo_dev, sizeof(ThermoDev));
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->own_stream, cudaStreamNonBlocking);
     if (e == cudaSuccess && prm.precision == GPUANN_PRECISION_BF16) e = gemm_setup(c);
+    if (e == cudaSuccess && prm.precision == GPUANN_PRECISION_BF16) e = fused_setup(c);
     if (e != cudaSuccess) {
         int rc = fail_cuda(nullptr, e, "gpuann_create");
         gpuann_destroy(c);
@@ -250,7 +254,12 @@ int gpuann_load_net(gpuann_ctx *c, int n_species, int n_layers, const int *sizes
     }
 
     // ---- BF16 tensor path: pad, round (RNE), upload, encode the tensor maps
-    int64_t chunk = c->prm.chunk_cells > 0 ? c->prm.chunk_cells : (int64_t)c->sm_count * 128;
+    // variant: "bf16-fused" (S1 + S2 + layers 1-2 in one kernel, k_fused.cu) when the shapes allow it, else
+    // "bf16-layerwise".  GPUANN_VARIANT=layerwise forces the latter (A/B measurements).
+    const char *force = std::getenv("GPUANN_VARIANT");
+    const bool want_fused = !(force && std::strcmp(force, "layerwise") == 0);
+    const bool fused = want_fused && n_layers >= 3 && fused_supported(sizes[0], sizes[1], pad16(sizes[2]));
+    int64_t chunk = c->prm.chunk_cells > 0 ? c->prm.chunk_cells : (int64_t)c->sm_count * 128 * (fused ? 16 : 1);
     chunk = (chunk + 127) / 128 * 128;
     c->chunk = chunk;
     int maxKp = 0;
@@ -264,7 +273,7 @@ int gpuann_load_net(gpuann_ctx *c, int n_species, int n_layers, const int *sizes
         ly.tiles_n = (ly.Np + 255) / 256;
         ly.n_tile = pad16((ly.Np + ly.tiles_n - 1) / ly.tiles_n);
         ly.tiles_n = (ly.Np + ly.n_tile - 1) / ly.n_tile;
-        maxKp = ly.Kp > maxKp ? ly.Kp : maxKp;
+        if (!fused || l >= 2) maxKp = ly.Kp > maxKp ? ly.Kp : maxKp;
         mac += (int64_t)ly.Kp * ly.Np;
         std::vector<uint16_t> hw((size_t)ly.Np * ly.Kp, 0);
         std::vector<float> hb((size_t)ly.Np, 0.f);
@@ -280,6 +289,38 @@ int gpuann_load_net(gpuann_ctx *c, int n_species, int n_layers, const int *sizes
         if (!encode_tmap_bf16(&ly.tmapW, ly.W, (uint64_t)ly.Kp, (uint64_t)ly.Np, (uint64_t)ly.Kp * 2, (uint32_t)ly.n_tile, &terr))
             return fail(c, GPUANN_ERR_CUDA, "gpuann_load_net: " + terr);
     }
+    if (fused) {
+        FusedNet &fn = c->fused;
+        const int D = sizes[0], H1 = sizes[1];
+        fused_plan(c->lay[1].Np, &fn.n_pass, &fn.pass_w, &fn.n0, &fn.n1);
+        // W1 padded to K = 64 with the bias in two extra columns: b1 = hi + lo, both BF16, multiplied by the
+        // constant-1 features z[D], z[D+1] the kernel appends (bias error <= 2^-17 |b1|)
+        std::vector<uint16_t> w1((size_t)H1 * 64, 0);
+        for (int j = 0; j < H1; ++j) {
+            for (int i = 0; i < D; ++i) w1[(size_t)j * 64 + i] = f32_to_bf16_rne(weights[0][(size_t)j * D + i]);
+            const float b = biases[0][j];
+            const uint16_t hi = f32_to_bf16_rne(b);
+            uint32_t hbits = (uint32_t)hi << 16;
+            float hf;
+            std::memcpy(&hf, &hbits, 4);
+            w1[(size_t)j * 64 + D] = hi;
+            w1[(size_t)j * 64 + D + 1] = f32_to_bf16_rne(b - hf);
+        }
+        CU_TRY(c, cudaMalloc(&fn.W1p, w1.size() * sizeof(uint16_t)), "cudaMalloc(W1 padded)");
+        CU_TRY(c, cudaMemcpy(fn.W1p, w1.data(), w1.size() * sizeof(uint16_t), cudaMemcpyHostToDevice), "cudaMemcpy(W1 padded)");
+        std::string terr;
+        const LayerBf16 &l2 = c->lay[1];
+        if (!encode_tmap_bf16(&fn.tmapW1, fn.W1p, 64, (uint64_t)H1, 128, 64, &terr) ||
+            !encode_tmap_bf16(&fn.tmapW2a, l2.W, (uint64_t)l2.Kp, (uint64_t)l2.Np, (uint64_t)l2.Kp * 2, (uint32_t)fn.n0, &terr) ||
+            !encode_tmap_bf16(&fn.tmapW2b, l2.W, (uint64_t)l2.Kp, (uint64_t)l2.Np, (uint64_t)l2.Kp * 2,
+                              (uint32_t)(fn.n1 > 0 ? fn.n1 : 16), &terr))
+            return fail(c, GPUANN_ERR_CUDA, "gpuann_load_net: " + terr);
+        fn.on = true;
+        // MACs issued: layer 1 once per pass over 16 * Kz columns, layer 2 over n_pass * pass_w columns
+        const int Kz16 = ((D + 2 + 15) / 16) * 16;
+        mac += (int64_t)fn.n_pass * H1 * Kz16 - (int64_t)c->lay[0].Kp * c->lay[0].Np;
+        mac += (int64_t)H1 * ((int64_t)fn.n_pass * fn.pass_w - l2.Np);
+    }
     c->act_elems = (size_t)chunk * (size_t)maxKp;
     for (int b = 0; b < 2; ++b) {
         CU_TRY(c, cudaMalloc(&c->act[b], c->act_elems * sizeof(__nv_bfloat16)), "cudaMalloc(activations)");
@@ -287,14 +328,14 @@ int gpuann_load_net(gpuann_ctx *c, int n_species, int n_layers, const int *sizes
     }
     CU_TRY(c, cudaMalloc(&c->o_buf, (size_t)n_species * chunk * sizeof(float)), "cudaMalloc(o_buf)");
     CU_TRY(c, cudaMemset(c->o_buf, 0, (size_t)n_species * chunk * sizeof(float)), "cudaMemset(o_buf)");
-    for (int l = 0; l < n_layers; ++l) {
+    for (int l = fused ? 2 : 0; l < n_layers; ++l) {
         LayerBf16 &ly = c->lay[l];
         std::string terr;
         if (!encode_tmap_bf16(&ly.tmapA, c->act[l & 1], (uint64_t)ly.Kp, (uint64_t)chunk, (uint64_t)ly.Kp * 2, 128, &terr))
             return fail(c, GPUANN_ERR_CUDA, "gpuann_load_net: " + terr);
     }
     c->issued_mac_per_cell = mac;
-    c->variant = "bf16-layerwise";
+    c->variant = fused ? "bf16-fused" : "bf16-layerwise";
     c->net_loaded = true;
     return GPUANN_OK;
 }
@@ -373,8 +414,14 @@ int ensure_compaction_scratch(Ctx *c, int64_t n) {
 // S1-S3 of the tensor path for the chunk [c0, c0+cn): z -> layers -> raw output o (FP32, [Ns][stride])
 int forward_chunk_bf16(Ctx *c, int64_t n, int64_t c0, int64_t cn, const float *T, const float *p, const float *Y,
                        bool use_idx, float *o, int64_t o_stride, cudaStream_t s) {
-    CU_TRY(c, launch_pre_bf16(c, n, c0, cn, T, p, Y, use_idx, c->act[0], c->lay[0].Kp, s), "pre kernel");
-    for (int l = 0; l < c->L; ++l) {
+    int l0 = 0;
+    if (c->fused.on) {
+        CU_TRY(c, launch_fused_l1l2(c, n, c0, cn, T, p, Y, use_idx, s), "fused kernel");
+        l0 = 2;
+    } else {
+        CU_TRY(c, launch_pre_bf16(c, n, c0, cn, T, p, Y, use_idx, c->act[0], c->lay[0].Kp, s), "pre kernel");
+    }
+    for (int l = l0; l < c->L; ++l) {
         const bool last = l == c->L - 1;
         __nv_bfloat16 *out = last ? nullptr : c->act[(l + 1) & 1];
         CU_TRY(c,

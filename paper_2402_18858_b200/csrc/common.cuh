@@ -72,6 +72,15 @@ struct LayerBf16 {
     CUtensorMap tmapA;   // this layer's input: activation buffer [chunk][Kp], box {64, 128}
 };
 
+// "bf16-fused" variant: S1 + S2 + layers 1-2 in one kernel (k_fused.cu)
+struct FusedNet {
+    bool on = false;
+    __nv_bfloat16 *W1p = nullptr;  // DEVICE [H1][64]: W1 zero padded to K = 64, b1 (hi, lo) in columns D, D+1
+    CUtensorMap tmapW1{};          // box {64, 64}
+    CUtensorMap tmapW2a{}, tmapW2b{};  // W2 [H2p][H1]: box {64, n0}, box {64, n1}
+    int n_pass = 0, pass_w = 0, n0 = 0, n1 = 0;
+};
+
 struct Ctx {
     gpuann_params prm{};
     int device = 0;
@@ -98,6 +107,7 @@ struct Ctx {
     float *o_buf = nullptr;                   // [Ns][chunk] raw output of the chunk
     int64_t issued_mac_per_cell = 0;
     const char *variant = "none";
+    FusedNet fused;
 
     // thermo
     bool thermo_loaded = false;
@@ -191,6 +201,13 @@ cudaError_t gemm_setup(Ctx *c);  // opt-in shared memory etc.
 cudaError_t launch_layer_bf16(Ctx *c, int layer, int64_t rows_cap, const CUtensorMap *tmapA, __nv_bfloat16 *out_bf16,
                               int out_ld, float *out_f32, int64_t out_f32_stride, int64_t c0, bool use_count,
                               cudaStream_t s);
+
+// k_fused.cu
+cudaError_t fused_setup(Ctx *c);
+bool fused_supported(int D, int H1, int H2p);
+void fused_plan(int H2p, int *n_pass, int *pass_w, int *n0, int *n1);
+cudaError_t launch_fused_l1l2(Ctx *c, int64_t n, int64_t c0, int64_t cn, const float *T, const float *p, const float *Y,
+                              bool use_idx, cudaStream_t s);
 
 // encodes a 2-D BF16 row-major tensor map {inner = cols, outer = rows}, box {64, box_rows}, 128-byte swizzle
 bool encode_tmap_bf16(CUtensorMap *out, const void *base, uint64_t cols, uint64_t rows, uint64_t row_pitch_bytes,

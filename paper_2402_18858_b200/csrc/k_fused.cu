@@ -5,20 +5,21 @@
 // Why: layer 2 holds 78 % of the FLOPs and its A operand h1 (3.2 KB/cell) is the largest
 // activation; producing it on the fly from the 64-byte z row removes the h1 round trip and leaves the weights
 // as the only L2 -> SMEM stream.  TMEM (512 columns) cannot hold a 128 x 800 FP32 accumulator, so the H2
-// columns are processed in n_pass passes of <= 416 columns and h1 is recomputed per pass (layer 1 is 2 % of
-// the FLOPs; its GELU runs on otherwise idle ALUs under the layer-2 MMAs).
+// columns are processed in n_pass passes of <= 416 columns and h1 is recomputed per pass.
 //
-// Roles (384 threads, one CTA per SM, tiles of 128 cells walked with stride gridDim.x):
+// Roles (512 threads, one CTA per SM, tiles of 128 cells walked with stride gridDim.x):
 //   warp 0      TMA: W2 k-block [pass_w x 64] ring of 2, W1 rows [64 x 64] ring of 4 (runs 2 chunks ahead)
-//   warp 1      tcgen05.mma issuer (one lane) + TMEM owner
-//                 L1: D = L1acc[slot] (128 x 32 FP32), A = z tile (smem), B = W1 rows; bias b1 rides in two
-//                     extra K columns of W1 against two constant-1 columns of z (hi + lo BF16 split)
-//                 L2: D = acc[0..pass_w), A = h1 chunk (smem, written by the producers), B = W2 k-block
-//   warps 2-3   z builder: state (SoA, gathered through idx when compaction is on) -> Box-Cox -> z-score ->
+//   warp 1      layer-2 tcgen05.mma issuer + TMEM owner:  acc[0..pass_w) += h1 chunk (smem) x W2 k-block
+//   warp 2      layer-1 tcgen05.mma issuer:  L1acc[slot] (128 x 32 FP32) = z tile (smem) x W1 rows; bias b1
+//               rides in two extra K columns of W1 against two constant-1 columns of z (hi + lo BF16 split)
+//   warp 3      z builder: state (SoA, gathered through idx when compaction is on) -> Box-Cox -> z-score ->
 //               BF16 -> 128-byte-swizzled smem tile, double buffered across tiles
-//   warps 4-11  producers / epilogue: tcgen05.ld of an L1 sub-chunk -> GELU -> BF16 -> swizzled A chunk;
-//               after a pass: tcgen05.ld of acc -> + b2 -> GELU -> BF16 -> smem staging -> coalesced 16-byte
-//               global stores of h2.
+//   warps 4-11  h1 producers: tcgen05.ld of an L1 sub-chunk -> GELU -> BF16 -> swizzled A chunk
+//   warps 12-15 pass epilogue: tcgen05.ld of acc -> + b2 -> GELU -> BF16 -> 64-byte row segments of h2 (global)
+// The two MMA warps run warp-uniform loops and predicate only the tcgen05 instructions on one lane: inside an
+// `if (lane == 0)` branch ptxas cannot use the uniform datapath and spends ~20 vector instructions + R2UR
+// per MMA, which made ONE thread the bottleneck of the first version of this kernel (465 SASS instructions
+// per 64-column chunk, ~3000 clk against 800 clk of MMA work; profiles/r01_fused_l1l2_v1.md).
 #include "common.cuh"
 #include "post.cuh"
 #include "ptx.cuh"
@@ -34,8 +35,7 @@ constexpr int kAStages = 3;
 constexpr int kL1Slots = 3;
 constexpr int kAccCols = 416;    // TMEM columns of the layer-2 accumulator (max pass width)
 constexpr int kL1Col = kAccCols; // L1 slots live in columns 416..511
-constexpr int kFusedThreads = 384;
-constexpr int kProdThreads = 256;
+constexpr int kFusedThreads = 512;
 
 constexpr uint32_t kW2StageBytes = kAccCols * 128;  // 53,248
 constexpr uint32_t kW1StageBytes = kFK * 128;       // 8,192
@@ -79,6 +79,17 @@ __device__ __forceinline__ float gelu_tanh_f(float v) {
     return fmaf(hv, ptx::tanh_approx(u), hv);
 }
 
+// ring position: stage index + phase bit, advanced without integer division
+struct Ring {
+    uint32_t st = 0, ph = 0;
+    __device__ __forceinline__ void next(uint32_t n) {
+        if (++st == n) {
+            st = 0;
+            ph ^= 1u;
+        }
+    }
+};
+
 __global__ void __launch_bounds__(kFusedThreads, 1)
 k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__ CUtensorMap tmapW2a,
              const __grid_constant__ CUtensorMap tmapW2b, const FusedArgs fa) {
@@ -99,16 +110,15 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
     const int n_tiles = (int)((rows + kFM - 1) / kFM);
     const int my_tiles = n_tiles > (int)blockIdx.x ? (n_tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
     const int n_chunks = fa.H1 / kFK;
-    const int n_sub = 2 * n_chunks;
 
     if (threadIdx.x == 0) {
         for (int i = 0; i < kW2Stages; ++i) { ptx::mbar_init(&bars[bW2Full + i], 1); ptx::mbar_init(&bars[bW2Empty + i], 1); }
         for (int i = 0; i < kW1Stages; ++i) { ptx::mbar_init(&bars[bW1Full + i], 1); ptx::mbar_init(&bars[bW1Empty + i], 1); }
         for (int i = 0; i < kAStages; ++i) { ptx::mbar_init(&bars[bAFull + i], 8); ptx::mbar_init(&bars[bAEmpty + i], 1); }
         for (int i = 0; i < kL1Slots; ++i) { ptx::mbar_init(&bars[bL1Full + i], 1); ptx::mbar_init(&bars[bL1Empty + i], 4); }
-        for (int i = 0; i < 2; ++i) { ptx::mbar_init(&bars[bZFull + i], 2); ptx::mbar_init(&bars[bZEmpty + i], 1); }
+        for (int i = 0; i < 2; ++i) { ptx::mbar_init(&bars[bZFull + i], 1); ptx::mbar_init(&bars[bZEmpty + i], 1); }
         ptx::mbar_init(&bars[bAccFull], 1);
-        ptx::mbar_init(&bars[bAccEmpty], 8);
+        ptx::mbar_init(&bars[bAccEmpty], 4);
         ptx::fence_mbar_init();
     }
     if (warp == 0 && lane == 0) {
@@ -125,110 +135,106 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
     __syncthreads();
     ptx::tc_fence_after_sync();
     const uint32_t tmem_base = *tmem_slot;
+    const uint32_t elected = lane == 0 ? 1u : 0u;
+    const uint64_t desc0 = ptx::umma_desc_sw128_kmajor(sbase);  // + (byte offset >> 4) addresses any tile below
 
     if (warp == 0) {
         // ================================================================ TMA: weights only (tile independent)
         if (lane == 0) {
-            const int per_tile = fa.n_pass * n_chunks;
-            const int64_t total = (int64_t)my_tiles * per_tile;
+            const int64_t total = (int64_t)my_tiles * fa.n_pass * n_chunks;
             const uint32_t w2_bytes = (uint32_t)(fa.n0 + fa.n1) * 128u;
+            Ring w1, w2;
+            int c1 = 0;           // chunk of the W1 sequence
+            int c2 = 0, p2 = 0;   // chunk / pass of the W2 sequence
             for (int64_t i = 0; i < total + 2; ++i) {
                 if (i < total) {
-                    const int st = (int)(i & (kW1Stages - 1));
-                    ptx::mbar_wait(&bars[bW1Empty + st], (uint32_t)((i / kW1Stages) & 1) ^ 1u);
-                    ptx::mbar_arrive_expect_tx(&bars[bW1Full + st], kW1StageBytes);
-                    ptx::tma_load_2d(&tmapW1, &bars[bW1Full + st], smem + kOffW1 + st * kW1StageBytes, 0,
-                                     (int)(i % n_chunks) * kFK);
+                    ptx::mbar_wait(&bars[bW1Empty + w1.st], w1.ph ^ 1u);
+                    ptx::mbar_arrive_expect_tx(&bars[bW1Full + w1.st], kW1StageBytes);
+                    ptx::tma_load_2d(&tmapW1, &bars[bW1Full + w1.st], smem + kOffW1 + w1.st * kW1StageBytes, 0, c1 * kFK);
+                    w1.next(kW1Stages);
+                    if (++c1 == n_chunks) c1 = 0;
                 }
                 if (i >= 2) {
-                    const int64_t j = i - 2;
-                    const int st = (int)(j % kW2Stages);
-                    const int chunk = (int)(j % n_chunks);
-                    const int pass = (int)((j / n_chunks) % fa.n_pass);
-                    ptx::mbar_wait(&bars[bW2Empty + st], (uint32_t)((j / kW2Stages) & 1) ^ 1u);
-                    ptx::mbar_arrive_expect_tx(&bars[bW2Full + st], w2_bytes);
-                    unsigned char *dst = smem + kOffW2 + st * kW2StageBytes;
-                    ptx::tma_load_2d(&tmapW2a, &bars[bW2Full + st], dst, chunk * kFK, pass * fa.pass_w);
+                    ptx::mbar_wait(&bars[bW2Empty + w2.st], w2.ph ^ 1u);
+                    ptx::mbar_arrive_expect_tx(&bars[bW2Full + w2.st], w2_bytes);
+                    unsigned char *dst = smem + kOffW2 + w2.st * kW2StageBytes;
+                    ptx::tma_load_2d(&tmapW2a, &bars[bW2Full + w2.st], dst, c2 * kFK, p2 * fa.pass_w);
                     if (fa.n1 > 0)
-                        ptx::tma_load_2d(&tmapW2b, &bars[bW2Full + st], dst + (size_t)fa.n0 * 128, chunk * kFK,
-                                         pass * fa.pass_w + fa.n0);
+                        ptx::tma_load_2d(&tmapW2b, &bars[bW2Full + w2.st], dst + (size_t)fa.n0 * 128, c2 * kFK,
+                                         p2 * fa.pass_w + fa.n0);
+                    w2.next(kW2Stages);
+                    if (++c2 == n_chunks) {
+                        c2 = 0;
+                        if (++p2 == fa.n_pass) p2 = 0;
+                    }
                 }
             }
         }
     } else if (warp == 1) {
-        // ================================================================ MMA issuer
-        if (lane == 0) {
-            const uint32_t idesc_l1 = ptx::umma_idesc_bf16_f32(kFM, kSub);
-            const uint32_t idesc_n0 = ptx::umma_idesc_bf16_f32(kFM, (uint32_t)fa.n0);
-            const uint32_t idesc_n1 = ptx::umma_idesc_bf16_f32(kFM, (uint32_t)(fa.n1 > 0 ? fa.n1 : 16));
-            uint32_t g1 = 0;   // L1 sub-chunks issued so far (ring of kL1Slots)
-            uint32_t gw = 0;   // chunk sequence number at the start of the current pass
-            uint32_t gc = 0;   // L2 chunks issued so far
-            uint32_t acc_use = 0;
-            for (int it = 0; it < my_tiles; ++it) {
-                const int zb = it & 1;
-                ptx::mbar_wait(&bars[bZFull + zb], (uint32_t)(it >> 1) & 1u);
+        // ================================================================ layer-2 MMA issuer (whole warp, uniform)
+        const uint32_t idesc_n0 = ptx::umma_idesc_bf16_f32(kFM, (uint32_t)fa.n0);
+        const uint32_t idesc_n1 = ptx::umma_idesc_bf16_f32(kFM, (uint32_t)(fa.n1 > 0 ? fa.n1 : 16));
+        const uint32_t n1_on = fa.n1 > 0 ? elected : 0u;
+        const uint64_t b1_off = (uint64_t)((uint32_t)fa.n0 * 128u >> 4);
+        Ring a, w2;
+        uint32_t acc_ph = 0;
+        for (int it = 0; it < my_tiles; ++it) {
+            for (int pass = 0; pass < fa.n_pass; ++pass) {
+                ptx::mbar_wait(&bars[bAccEmpty], acc_ph ^ 1u);
                 ptx::tc_fence_after_sync();
-                const uint32_t z_addr = sbase + kOffZ + zb * kZBytes;
-                for (int pass = 0; pass < fa.n_pass; ++pass) {
-                    ptx::mbar_wait(&bars[bAccEmpty], (acc_use & 1u) ^ 1u);
+                for (int c = 0; c < n_chunks; ++c) {
+                    ptx::mbar_wait(&bars[bW2Full + w2.st], w2.ph);
+                    ptx::mbar_wait(&bars[bAFull + a.st], a.ph);
                     ptx::tc_fence_after_sync();
-                    auto issue_l1 = [&](int s) {
-                        const uint32_t cw = gw + (uint32_t)(s >> 1);
-                        const int wst = (int)(cw % kW1Stages);
-                        if ((s & 1) == 0) {
-                            ptx::mbar_wait(&bars[bW1Full + wst], (cw / kW1Stages) & 1u);
-                            ptx::tc_fence_after_sync();
-                        }
-                        const int slot = (int)(g1 % kL1Slots);
-                        ptx::mbar_wait(&bars[bL1Empty + slot], ((g1 / kL1Slots) & 1u) ^ 1u);
-                        ptx::tc_fence_after_sync();
-                        const uint32_t b_addr = sbase + kOffW1 + wst * kW1StageBytes + (uint32_t)(s & 1) * (kSub * 128);
-                        const uint32_t d_tmem = tmem_base + kL1Col + (uint32_t)slot * kSub;
-                        for (int k = 0; k < fa.Kz; ++k)
-                            ptx::umma_bf16_ss(d_tmem, ptx::umma_desc_sw128_kmajor(z_addr + k * 32),
-                                              ptx::umma_desc_sw128_kmajor(b_addr + k * 32), idesc_l1, k ? 1u : 0u);
-                        ptx::umma_commit(&bars[bL1Full + slot]);
-                        ++g1;
-                    };
-                    issue_l1(0);
-                    issue_l1(1);
-                    for (int c = 0; c < n_chunks; ++c) {
-                        if (c + 1 < n_chunks) {
-                            issue_l1(2 * c + 2);
-                            issue_l1(2 * c + 3);
-                        }
-                        const int ast = (int)(gc % kAStages), wst2 = (int)(gc % kW2Stages);
-                        ptx::mbar_wait(&bars[bW2Full + wst2], (gc / kW2Stages) & 1u);
-                        ptx::mbar_wait(&bars[bAFull + ast], (gc / kAStages) & 1u);
-                        ptx::tc_fence_after_sync();
-                        const uint32_t a_addr = sbase + kOffA + ast * kAStageBytes;
-                        const uint32_t b_addr = sbase + kOffW2 + wst2 * kW2StageBytes;
+                    const uint64_t da = desc0 + (uint64_t)((kOffA + a.st * kAStageBytes) >> 4);
+                    const uint64_t db = desc0 + (uint64_t)((kOffW2 + w2.st * kW2StageBytes) >> 4);
 #pragma unroll
-                        for (int k = 0; k < kFK / 16; ++k) {
-                            const uint64_t da = ptx::umma_desc_sw128_kmajor(a_addr + k * 32);
-                            ptx::umma_bf16_ss(tmem_base, da, ptx::umma_desc_sw128_kmajor(b_addr + k * 32), idesc_n0,
-                                              (c | k) ? 1u : 0u);
-                            if (fa.n1 > 0)
-                                ptx::umma_bf16_ss(tmem_base + (uint32_t)fa.n0, da,
-                                                  ptx::umma_desc_sw128_kmajor(b_addr + (uint32_t)fa.n0 * 128 + k * 32),
-                                                  idesc_n1, (c | k) ? 1u : 0u);
-                        }
-                        ptx::umma_commit(&bars[bAEmpty + ast]);
-                        ptx::umma_commit(&bars[bW2Empty + wst2]);
-                        ptx::umma_commit(&bars[bW1Empty + (int)((gw + (uint32_t)c) % kW1Stages)]);
-                        ++gc;
+                    for (int k = 0; k < kFK / 16; ++k) {
+                        const uint32_t accum = (c | k) ? 1u : 0u;
+                        ptx::umma_bf16_ss_pred(tmem_base, da + 2 * k, db + 2 * k, idesc_n0, accum, elected);
+                        ptx::umma_bf16_ss_pred(tmem_base + (uint32_t)fa.n0, da + 2 * k, db + b1_off + 2 * k, idesc_n1, accum, n1_on);
                     }
-                    if (pass == fa.n_pass - 1) ptx::umma_commit(&bars[bZEmpty + zb]);
-                    ptx::umma_commit(&bars[bAccFull]);
-                    gw += (uint32_t)n_chunks;
-                    ++acc_use;
+                    ptx::umma_commit_pred(&bars[bAEmpty + a.st], elected);
+                    ptx::umma_commit_pred(&bars[bW2Empty + w2.st], elected);
+                    a.next(kAStages);
+                    w2.next(kW2Stages);
                 }
+                ptx::umma_commit_pred(&bars[bAccFull], elected);
+                acc_ph ^= 1u;
             }
         }
-    } else if (warp < 4) {
-        // ================================================================ z builder (64 threads, 2 cells each)
-        const int zt = (int)threadIdx.x - 64;
+    } else if (warp == 2) {
+        // ================================================================ layer-1 MMA issuer (whole warp, uniform)
+        const uint32_t idesc_l1 = ptx::umma_idesc_bf16_f32(kFM, kSub);
+        Ring w1, slot;
+        for (int it = 0; it < my_tiles; ++it) {
+            const uint32_t zb = (uint32_t)it & 1u;
+            ptx::mbar_wait(&bars[bZFull + zb], ((uint32_t)it >> 1) & 1u);
+            ptx::tc_fence_after_sync();
+            const uint64_t dz = desc0 + (uint64_t)((kOffZ + zb * kZBytes) >> 4);
+            for (int pass = 0; pass < fa.n_pass; ++pass) {
+                for (int c = 0; c < n_chunks; ++c) {
+                    ptx::mbar_wait(&bars[bW1Full + w1.st], w1.ph);
+                    const uint64_t dw = desc0 + (uint64_t)((kOffW1 + w1.st * kW1StageBytes) >> 4);
+#pragma unroll
+                    for (int s = 0; s < 2; ++s) {
+                        ptx::mbar_wait(&bars[bL1Empty + slot.st], slot.ph ^ 1u);
+                        ptx::tc_fence_after_sync();
+                        const uint32_t d_tmem = tmem_base + kL1Col + slot.st * kSub;
+                        const uint64_t dws = dw + (uint64_t)(s * ((kSub * 128) >> 4));
+                        for (int k = 0; k < fa.Kz; ++k)
+                            ptx::umma_bf16_ss_pred(d_tmem, dz + 2 * k, dws + 2 * k, idesc_l1, k ? 1u : 0u, elected);
+                        ptx::umma_commit_pred(&bars[bL1Full + slot.st], elected);
+                        slot.next(kL1Slots);
+                    }
+                    ptx::umma_commit_pred(&bars[bW1Empty + w1.st], elected);
+                    w1.next(kW1Stages);
+                }
+            }
+            ptx::umma_commit_pred(&bars[bZEmpty + zb], elected);
+        }
+    } else if (warp == 3) {
+        // ================================================================ z builder (32 threads, 4 cells each)
         const int D = fa.D;
         const int n_units = 2 * fa.Kz;  // 16-byte units (8 features) that carry data
         for (int it = 0; it < my_tiles; ++it) {
@@ -237,12 +243,13 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
             ptx::mbar_wait(&bars[bZEmpty + zb], ((uint32_t)(it >> 1) & 1u) ^ 1u);
             const uint32_t z_addr = sbase + kOffZ + zb * kZBytes;
 #pragma unroll 1
-            for (int rr = zt; rr < kFM; rr += 64) {
+            for (int rr = lane; rr < kFM; rr += 32) {
                 const int64_t i = (int64_t)tile * kFM + rr;
                 const bool valid = i < rows;
                 int64_t g = fa.c0 + i;
                 if (fa.idx) g = valid ? (int64_t)fa.idx[g] : 0;
                 const uint32_t row_addr = z_addr + (uint32_t)rr * 128u;
+#pragma unroll 1
                 for (int u = 0; u < 8; ++u) {
                     float v[8];
 #pragma unroll
@@ -254,8 +261,14 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
                                 if (j == 0) x = fa.T[g];
                                 else if (j == 1) x = fa.p[g];
                                 else {
+                                    // z is rounded to BF16 (2^-9): the approximate lg2 / ex2 pair (2^-22) is ample here;
+                                    // Y = 0 still maps to exactly -1/lambda (R1, R2)
                                     const float Yc = fmaxf(fa.Y[(int64_t)(j - 2) * fa.n + g], 0.f);
-                                    x = boxcox_y(Yc, boxcox_u(Yc, fa.pre.lambda), fa.pre);
+                                    if (fa.pre.lambda_zero) x = logf(Yc);
+                                    else {
+                                        const float uu = Yc > 0.f ? ptx::ex2_approx(fa.pre.lambda * ptx::lg2_approx(Yc)) : 0.f;
+                                        x = (uu - 1.f) * fa.pre.inv_lambda;
+                                    }
                                 }
                                 x = (x - fa.pre.mean[j]) * fa.pre.inv_std[j];
                             } else if (j < D + 2) {
@@ -273,110 +286,105 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
             __syncwarp();
             if (lane == 0) ptx::mbar_arrive(&bars[bZFull + zb]);
         }
-    } else {
-        // ================================================================ producers / epilogue (warps 4..11)
+    } else if (warp < 12) {
+        // ================================================================ h1 producers (warps 4..11)
         const int q = warp & 3;             // TMEM lane quarter
-        const int set = (warp - 4) >> 2;    // which 32-column half of a 64-column chunk / piece
+        const int set = (warp - 4) >> 2;    // which 32-column half of a 64-column chunk
         const int r = q * 32 + lane;        // row of the tile
-        const int pt = (int)threadIdx.x - 128;  // 0..255
-        const uint32_t lane_addr = tmem_base + ((uint32_t)(q * 32) << 16);
+        const uint32_t lane_addr = tmem_base + ((uint32_t)(q * 32) << 16) + kL1Col;
         const uint32_t swz = (uint32_t)(r & 7);
-        uint32_t gsub = 0, gch = 0, acc_use = 0;
+        const uint32_t row_off = (uint32_t)r * 128u;
+        uint32_t slot = (uint32_t)set, slot_ph = 0;  // sub-chunk g = 2 c + set lives in slot g % 3, phase (g / 3) & 1
+        Ring a;
+        const int total_chunks = my_tiles * fa.n_pass * n_chunks;
+#pragma unroll 1
+        for (int c = 0; c < total_chunks; ++c) {
+            ptx::mbar_wait(&bars[bL1Full + slot], slot_ph);
+            ptx::tc_fence_after_sync();
+            uint32_t v[32];
+            ptx::tmem_ld32(lane_addr + slot * kSub, v);
+            ptx::tmem_ld_wait();
+            ptx::tc_fence_before_sync();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(&bars[bL1Empty + slot]);
+            uint32_t o[16];
+#pragma unroll
+            for (int j = 0; j < 16; ++j)
+                o[j] = ptx::pack_bf16x2(gelu_tanh_f(__uint_as_float(v[2 * j])), gelu_tanh_f(__uint_as_float(v[2 * j + 1])));
+            ptx::mbar_wait(&bars[bAEmpty + a.st], a.ph ^ 1u);
+            const uint32_t row_addr = sbase + kOffA + a.st * kAStageBytes + row_off;
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+                ptx::st_shared_v4(row_addr + ((((uint32_t)(4 * set + i)) ^ swz) << 4), o[4 * i], o[4 * i + 1],
+                                  o[4 * i + 2], o[4 * i + 3]);
+            ptx::fence_proxy_async_smem();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(&bars[bAFull + a.st]);
+            a.next(kAStages);
+            slot += 2;
+            if (slot >= kL1Slots) {
+                slot -= kL1Slots;
+                slot_ph ^= 1u;
+            }
+        }
+    } else {
+        // ================================================================ pass epilogue (warps 12..15)
+        const int q = warp & 3;
+        const int r = q * 32 + lane;
+        const uint32_t lane_addr = tmem_base + ((uint32_t)(q * 32) << 16);
+        uint32_t acc_ph = 0;
         for (int it = 0; it < my_tiles; ++it) {
             const int tile = (int)blockIdx.x + it * (int)gridDim.x;
+            const int64_t grow = (int64_t)tile * kFM + r;
+            const bool row_ok = grow < rows;
             for (int pass = 0; pass < fa.n_pass; ++pass) {
-                // ---------------- h1 sub-chunks of this warp set
-                for (int s = set; s < n_sub; s += 2) {
-                    const uint32_t g = gsub + (uint32_t)s;
-                    const int slot = (int)(g % kL1Slots);
-                    ptx::mbar_wait(&bars[bL1Full + slot], (g / kL1Slots) & 1u);
-                    ptx::tc_fence_after_sync();
-                    uint32_t v[32];
-                    ptx::tmem_ld32(lane_addr + kL1Col + (uint32_t)slot * kSub, v);
-                    ptx::tmem_ld_wait();
-                    ptx::tc_fence_before_sync();
-                    __syncwarp();
-                    if (lane == 0) ptx::mbar_arrive(&bars[bL1Empty + slot]);
-                    uint32_t o[16];
-#pragma unroll
-                    for (int j = 0; j < 16; ++j)
-                        o[j] = ptx::pack_bf16x2(gelu_tanh_f(__uint_as_float(v[2 * j])),
-                                                gelu_tanh_f(__uint_as_float(v[2 * j + 1])));
-                    const uint32_t gc = gch + (uint32_t)(s >> 1);
-                    const int ast = (int)(gc % kAStages);
-                    ptx::mbar_wait(&bars[bAEmpty + ast], ((gc / kAStages) & 1u) ^ 1u);
-                    const uint32_t row_addr = sbase + kOffA + ast * kAStageBytes + (uint32_t)r * 128u;
-#pragma unroll
-                    for (int i = 0; i < 4; ++i)
-                        ptx::st_shared_v4(row_addr + ((((uint32_t)(4 * set + i)) ^ swz) << 4), o[4 * i], o[4 * i + 1],
-                                          o[4 * i + 2], o[4 * i + 3]);
-                    ptx::fence_proxy_async_smem();
-                    __syncwarp();
-                    if (lane == 0) ptx::mbar_arrive(&bars[bAFull + ast]);
-                }
-                gsub += (uint32_t)n_sub;
-                gch += (uint32_t)n_chunks;
-
-                // ---------------- epilogue of the pass: acc -> + b2 -> GELU -> BF16 -> staging -> global
-                ptx::mbar_wait(&bars[bAccFull], acc_use & 1u);
+                ptx::mbar_wait(&bars[bAccFull], acc_ph);
                 ptx::tc_fence_after_sync();
-                ++acc_use;
+                acc_ph ^= 1u;
                 const int col_base = pass * fa.pass_w;
                 int cur_w = fa.H2p - col_base;
                 cur_w = cur_w < fa.pass_w ? cur_w : fa.pass_w;
-                const int n_pieces = (cur_w + kFK - 1) / kFK;
-                // last piece in which this warp set still reads the accumulator (-1: it reads nothing)
-                const int last_pc = cur_w > set * kSub ? (cur_w - set * kSub - 1) / kFK : -1;
-                if (last_pc < 0) {
-                    __syncwarp();
-                    if (lane == 0) ptx::mbar_arrive(&bars[bAccEmpty]);
-                }
-                for (int pc = 0; pc < n_pieces; ++pc) {
-                    const int col_lo = pc * kFK + set * kSub;  // within the pass
-                    const uint32_t stage_addr = sbase + kOffA + (uint32_t)(pc % kAStages) * kAStageBytes;
-                    if (col_lo < cur_w) {
-                        uint32_t v[32];
-                        ptx::tmem_ld32(lane_addr + (uint32_t)col_lo, v);
-                        ptx::tmem_ld_wait();
-                        if (pc == last_pc) {
-                            // last accumulator read of this warp: hand the accumulator back to the MMA warp
-                            ptx::tc_fence_before_sync();
-                            __syncwarp();
-                            if (lane == 0) ptx::mbar_arrive(&bars[bAccEmpty]);
-                        }
-                        const float4 *b4 = reinterpret_cast<const float4 *>(sBias + col_base + col_lo);
-                        uint32_t o[16];
+                __nv_bfloat16 *dst_row = fa.h2 + grow * fa.H2p + col_base;
+#pragma unroll 1
+                for (int cc = 0; cc < cur_w; cc += 32) {
+                    const bool full = cc + 32 <= cur_w;  // widths are multiples of 16: the tail piece has 16 columns
+                    uint32_t v[32];
+                    if (full) ptx::tmem_ld32(lane_addr + (uint32_t)cc, v);
+                    else {
+                        uint32_t w[16];
+                        ptx::tmem_ld16(lane_addr + (uint32_t)cc, w);
 #pragma unroll
-                        for (int j = 0; j < 8; ++j) {
-                            const float4 b = b4[j];
-                            o[2 * j] = ptx::pack_bf16x2(gelu_tanh_f(__uint_as_float(v[4 * j]) + b.x),
-                                                        gelu_tanh_f(__uint_as_float(v[4 * j + 1]) + b.y));
-                            o[2 * j + 1] = ptx::pack_bf16x2(gelu_tanh_f(__uint_as_float(v[4 * j + 2]) + b.z),
-                                                            gelu_tanh_f(__uint_as_float(v[4 * j + 3]) + b.w));
-                        }
-                        const uint32_t row_addr = stage_addr + (uint32_t)r * 128u;
+                        for (int j = 0; j < 16; ++j) v[j] = w[j];
 #pragma unroll
-                        for (int i = 0; i < 4; ++i)
-                            ptx::st_shared_v4(row_addr + ((((uint32_t)(4 * set + i)) ^ swz) << 4), o[4 * i],
-                                              o[4 * i + 1], o[4 * i + 2], o[4 * i + 3]);
+                        for (int j = 16; j < 32; ++j) v[j] = 0u;
                     }
-                    ptx::named_bar_sync(1, kProdThreads);
-                    // copy the 128 x 64 piece out: unit = 16 bytes = 8 columns; a warp covers 4 rows x 128 bytes
+                    ptx::tmem_ld_wait();
+                    if (cc + 32 >= cur_w) {
+                        // last accumulator read of this warp: hand the accumulator back to the MMA warp
+                        ptx::tc_fence_before_sync();
+                        __syncwarp();
+                        if (lane == 0) ptx::mbar_arrive(&bars[bAccEmpty]);
+                    }
+                    const float4 *b4 = reinterpret_cast<const float4 *>(sBias + col_base + cc);
+                    uint32_t o[16];
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        const int unit = pt + i * kProdThreads;
-                        const int row = unit >> 3, u = unit & 7;
-                        const int col = pc * kFK + u * 8;
-                        const int64_t grow = (int64_t)tile * kFM + row;
-                        if (col < cur_w && grow < rows) {
-                            const uint4 val = ptx::ld_shared_v4(stage_addr + (uint32_t)row * 128u + (uint32_t)((u ^ (row & 7)) << 4));
-                            *reinterpret_cast<uint4 *>(fa.h2 + grow * fa.H2p + col_base + col) = val;
+                    for (int j = 0; j < 8; ++j) {
+                        const float4 b = (full || j < 4) ? b4[j] : make_float4(0.f, 0.f, 0.f, 0.f);
+                        o[2 * j] = ptx::pack_bf16x2(gelu_tanh_f(__uint_as_float(v[4 * j]) + b.x),
+                                                    gelu_tanh_f(__uint_as_float(v[4 * j + 1]) + b.y));
+                        o[2 * j + 1] = ptx::pack_bf16x2(gelu_tanh_f(__uint_as_float(v[4 * j + 2]) + b.z),
+                                                        gelu_tanh_f(__uint_as_float(v[4 * j + 3]) + b.w));
+                    }
+                    if (row_ok) {
+                        uint4 *dst = reinterpret_cast<uint4 *>(dst_row + cc);
+                        dst[0] = make_uint4(o[0], o[1], o[2], o[3]);
+                        dst[1] = make_uint4(o[4], o[5], o[6], o[7]);
+                        if (full) {
+                            dst[2] = make_uint4(o[8], o[9], o[10], o[11]);
+                            dst[3] = make_uint4(o[12], o[13], o[14], o[15]);
                         }
                     }
                 }
-                // staging aliases the A stages: nobody may start the next pass's producer stores before every
-                // thread has finished reading the last piece
-                ptx::named_bar_sync(1, kProdThreads);
             }
         }
     }
@@ -388,7 +396,6 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
         ptx::tmem_dealloc(tmem_base, 512);
     }
 }
-
 // ---------------------------------------------------------------- host side
 cudaError_t fused_setup(Ctx *c) {
     (void)c;

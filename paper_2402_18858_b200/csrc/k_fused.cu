@@ -242,44 +242,64 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
             const int zb = it & 1;
             ptx::mbar_wait(&bars[bZEmpty + zb], ((uint32_t)(it >> 1) & 1u) ^ 1u);
             const uint32_t z_addr = sbase + kOffZ + zb * kZBytes;
-#pragma unroll 1
-            for (int rr = lane; rr < kFM; rr += 32) {
-                const int64_t i = (int64_t)tile * kFM + rr;
-                const bool valid = i < rows;
-                int64_t g = fa.c0 + i;
-                if (fa.idx) g = valid ? (int64_t)fa.idx[g] : 0;
-                const uint32_t row_addr = z_addr + (uint32_t)rr * 128u;
-#pragma unroll 1
-                for (int u = 0; u < 8; ++u) {
-                    float v[8];
+            // 4 rows per lane (rr = lane + 32 q).  Loads first, arithmetic after: the 32 independent loads of a
+            // unit (8 features x 4 rows) are in flight together -- one memory latency per unit instead of one per
+            // load (the first version waited for every load in turn and needed ~100k clk per tile)
+            int64_t g4[4];
+            bool ok4[4];
 #pragma unroll
-                    for (int q = 0; q < 8; ++q) {
-                        const int j = u * 8 + q;
-                        float x = 0.f;
-                        if (valid && u < n_units) {
-                            if (j < D) {
-                                if (j == 0) x = fa.T[g];
-                                else if (j == 1) x = fa.p[g];
-                                else {
-                                    // z is rounded to BF16 (2^-9): the approximate lg2 / ex2 pair (2^-22) is ample here;
-                                    // Y = 0 still maps to exactly -1/lambda (R1, R2)
-                                    const float Yc = fmaxf(fa.Y[(int64_t)(j - 2) * fa.n + g], 0.f);
-                                    if (fa.pre.lambda_zero) x = logf(Yc);
-                                    else {
-                                        const float uu = Yc > 0.f ? ptx::ex2_approx(fa.pre.lambda * ptx::lg2_approx(Yc)) : 0.f;
-                                        x = (uu - 1.f) * fa.pre.inv_lambda;
-                                    }
-                                }
-                                x = (x - fa.pre.mean[j]) * fa.pre.inv_std[j];
-                            } else if (j < D + 2) {
-                                x = 1.f;  // multiplies the hi / lo halves of b1 stored in W1 columns D, D+1
-                            }
-                        }
-                        v[q] = x;
+            for (int q = 0; q < 4; ++q) {
+                const int64_t i = (int64_t)tile * kFM + lane + 32 * q;
+                ok4[q] = i < rows;
+                int64_t g = fa.c0 + i;
+                if (fa.idx) g = ok4[q] ? (int64_t)fa.idx[g] : 0;
+                g4[q] = ok4[q] ? g : 0;
+            }
+#pragma unroll 1
+            for (int u = 0; u < 8; ++u) {
+                float x[4][8];
+                if (u < n_units) {
+#pragma unroll
+                    for (int f = 0; f < 8; ++f) {
+                        const int j = u * 8 + f;
+                        const float *src = j == 0 ? fa.T : (j == 1 ? fa.p : fa.Y + (int64_t)(j - 2) * fa.n);
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) x[q][f] = (j < D && ok4[q]) ? src[g4[q]] : 0.f;
                     }
-                    ptx::st_shared_v4(row_addr + (uint32_t)((u ^ (rr & 7)) << 4), ptx::pack_bf16x2(v[0], v[1]),
-                                      ptx::pack_bf16x2(v[2], v[3]), ptx::pack_bf16x2(v[4], v[5]),
-                                      ptx::pack_bf16x2(v[6], v[7]));
+#pragma unroll
+                    for (int f = 0; f < 8; ++f) {
+                        const int j = u * 8 + f;
+                        const float mu = j < D ? fa.pre.mean[j] : 0.f, is = j < D ? fa.pre.inv_std[j] : 0.f;
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) {
+                            float t = x[q][f];
+                            if (j >= 2 && j < D) {
+                                // z is rounded to BF16 (2^-9): the approximate lg2 / ex2 pair (2^-22) is ample here;
+                                // Y = 0 still maps to exactly -1/lambda (R1, R2)
+                                const float Yc = fmaxf(t, 0.f);
+                                if (fa.pre.lambda_zero) t = logf(Yc);
+                                else {
+                                    const float uu = Yc > 0.f ? ptx::ex2_approx(fa.pre.lambda * ptx::lg2_approx(Yc)) : 0.f;
+                                    t = (uu - 1.f) * fa.pre.inv_lambda;
+                                }
+                            }
+                            t = (t - mu) * is;
+                            if (j >= D && j < D + 2) t = 1.f;  // multiplies the hi / lo halves of b1 in W1 columns D, D+1
+                            x[q][f] = ok4[q] ? t : 0.f;
+                        }
+                    }
+                } else {
+#pragma unroll
+                    for (int q = 0; q < 4; ++q)
+#pragma unroll
+                        for (int f = 0; f < 8; ++f) x[q][f] = 0.f;
+                }
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const int rr = lane + 32 * q;
+                    ptx::st_shared_v4(z_addr + (uint32_t)rr * 128u + (uint32_t)((u ^ (rr & 7)) << 4),
+                                      ptx::pack_bf16x2(x[q][0], x[q][1]), ptx::pack_bf16x2(x[q][2], x[q][3]),
+                                      ptx::pack_bf16x2(x[q][4], x[q][5]), ptx::pack_bf16x2(x[q][6], x[q][7]));
                 }
             }
             ptx::fence_proxy_async_smem();

@@ -135,7 +135,7 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
     __syncthreads();
     ptx::tc_fence_after_sync();
     const uint32_t tmem_base = *tmem_slot;
-    const uint32_t elected = lane == 0 ? 1u : 0u;
+
     const uint64_t desc0 = ptx::umma_desc_sw128_kmajor(sbase);  // + (byte offset >> 4) addresses any tile below
 
     if (warp == 0) {
@@ -174,7 +174,7 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
         // ================================================================ layer-2 MMA issuer (whole warp, uniform)
         const uint32_t idesc_n0 = ptx::umma_idesc_bf16_f32(kFM, (uint32_t)fa.n0);
         const uint32_t idesc_n1 = ptx::umma_idesc_bf16_f32(kFM, (uint32_t)(fa.n1 > 0 ? fa.n1 : 16));
-        const uint32_t n1_on = fa.n1 > 0 ? elected : 0u;
+
         const uint64_t b1_off = (uint64_t)((uint32_t)fa.n0 * 128u >> 4);
         Ring a, w2;
         uint32_t acc_ph = 0;
@@ -188,18 +188,23 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
                     ptx::tc_fence_after_sync();
                     const uint64_t da = desc0 + (uint64_t)((kOffA + a.st * kAStageBytes) >> 4);
                     const uint64_t db = desc0 + (uint64_t)((kOffW2 + w2.st * kW2StageBytes) >> 4);
+                    if (ptx::elect_one()) {
 #pragma unroll
-                    for (int k = 0; k < kFK / 16; ++k) {
-                        const uint32_t accum = (c | k) ? 1u : 0u;
-                        ptx::umma_bf16_ss_pred(tmem_base, da + 2 * k, db + 2 * k, idesc_n0, accum, elected);
-                        ptx::umma_bf16_ss_pred(tmem_base + (uint32_t)fa.n0, da + 2 * k, db + b1_off + 2 * k, idesc_n1, accum, n1_on);
+                        for (int k = 0; k < kFK / 16; ++k) {
+                            const uint32_t accum = (c | k) ? 1u : 0u;
+                            ptx::umma_bf16_ss(tmem_base, da + 2 * k, db + 2 * k, idesc_n0, accum);
+                            if (fa.n1 > 0)
+                                ptx::umma_bf16_ss(tmem_base + (uint32_t)fa.n0, da + 2 * k, db + b1_off + 2 * k, idesc_n1, accum);
+                        }
+                        ptx::umma_commit(&bars[bAEmpty + a.st]);
+                        ptx::umma_commit(&bars[bW2Empty + w2.st]);
                     }
-                    ptx::umma_commit_pred(&bars[bAEmpty + a.st], elected);
-                    ptx::umma_commit_pred(&bars[bW2Empty + w2.st], elected);
+                    __syncwarp();
                     a.next(kAStages);
                     w2.next(kW2Stages);
                 }
-                ptx::umma_commit_pred(&bars[bAccFull], elected);
+                if (ptx::elect_one()) ptx::umma_commit(&bars[bAccFull]);
+                __syncwarp();
                 acc_ph ^= 1u;
             }
         }
@@ -222,16 +227,21 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
                         ptx::tc_fence_after_sync();
                         const uint32_t d_tmem = tmem_base + kL1Col + slot.st * kSub;
                         const uint64_t dws = dw + (uint64_t)(s * ((kSub * 128) >> 4));
-                        for (int k = 0; k < fa.Kz; ++k)
-                            ptx::umma_bf16_ss_pred(d_tmem, dz + 2 * k, dws + 2 * k, idesc_l1, k ? 1u : 0u, elected);
-                        ptx::umma_commit_pred(&bars[bL1Full + slot.st], elected);
+                        if (ptx::elect_one()) {
+                            for (int k = 0; k < fa.Kz; ++k)
+                                ptx::umma_bf16_ss(d_tmem, dz + 2 * k, dws + 2 * k, idesc_l1, k ? 1u : 0u);
+                            ptx::umma_commit(&bars[bL1Full + slot.st]);
+                        }
+                        __syncwarp();
                         slot.next(kL1Slots);
                     }
-                    ptx::umma_commit_pred(&bars[bW1Empty + w1.st], elected);
+                    if (ptx::elect_one()) ptx::umma_commit(&bars[bW1Empty + w1.st]);
+                    __syncwarp();
                     w1.next(kW1Stages);
                 }
             }
-            ptx::umma_commit_pred(&bars[bZEmpty + zb], elected);
+            if (ptx::elect_one()) ptx::umma_commit(&bars[bZEmpty + zb]);
+            __syncwarp();
         }
     } else if (warp == 3) {
         // ================================================================ z builder (32 threads, 4 cells each)

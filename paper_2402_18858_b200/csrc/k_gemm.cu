@@ -5,7 +5,7 @@
 //   warp 1    allocates TMEM (512 columns = 2 accumulators of <= 256 columns) and issues tcgen05.mma
 //             (M = 128, N = n_tile, K = 16), committing each stage back to the producer and each finished
 //             accumulator to the epilogue
-//   warps 2-5 epilogue: tcgen05.ld 32 lanes x 16 columns, + bias, GELU, BF16 pack, 2 x 16-byte stores per row
+//   warps 2-9 epilogue (two per TMEM lane quarter): tcgen05.ld 32 lanes x 32 columns, + bias (smem), GELU, BF16 pack, 64-byte row segments
 //             (hidden layers) or FP32 species-major stores (last layer); overlaps the next tile's MMAs.
 // Tiles are walked n-fastest so that CTAs running together share the A rows and the whole W in L2.
 #include "common.cuh"
@@ -17,10 +17,11 @@ constexpr int kBM = 128;
 constexpr int kBK = 64;
 constexpr int kStages = 4;
 constexpr int kMaxNT = 256;
-constexpr int kGemmThreads = 192;
+constexpr int kGemmThreads = 320;   // TMA, MMA, 8 epilogue warps
 constexpr uint32_t kABytes = kBM * kBK * 2;        // 16 KB
 constexpr uint32_t kBBytesMax = kMaxNT * kBK * 2;  // 32 KB
-constexpr size_t kGemmSmem = 1024 /*align slack*/ + (size_t)kStages * (kABytes + kBBytesMax) + 256;
+constexpr int kBiasMax = 4096;  // = GPUANN_MAX_WIDTH floats staged in shared memory
+constexpr size_t kGemmSmem = 1024 /*align slack*/ + (size_t)kStages * (kABytes + kBBytesMax) + 256 + kBiasMax * 4;
 
 // GELU in the tanh form, tanh.approx.f32 (R5: any evaluation inside the BF16 tolerances)
 __device__ __forceinline__ float gelu_tanh(float v) {
@@ -52,6 +53,7 @@ k_layer_bf16(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ 
     uint64_t *bars = reinterpret_cast<uint64_t *>(sB + (size_t)kStages * kBBytesMax);
     uint64_t *full = bars, *empty = bars + kStages, *tfull = bars + 2 * kStages, *tempty = bars + 2 * kStages + 2;
     uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(bars + 2 * kStages + 4);
+    float *sBias = reinterpret_cast<float *>(sB + (size_t)kStages * kBBytesMax + 256);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -72,7 +74,7 @@ k_layer_bf16(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ 
         }
         for (int a = 0; a < 2; ++a) {
             ptx::mbar_init(&tfull[a], 1);
-            ptx::mbar_init(&tempty[a], 4);
+            ptx::mbar_init(&tempty[a], 8);
         }
         ptx::fence_mbar_init();
     }
@@ -84,6 +86,7 @@ k_layer_bf16(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ 
         ptx::tmem_alloc(tmem_slot, 512);
         ptx::tmem_relinquish();
     }
+    for (int i = threadIdx.x; i < ga.Np && i < kBiasMax; i += kGemmThreads) sBias[i] = ga.bias[i];
     ptx::tc_fence_before_sync();
     __syncthreads();
     ptx::tc_fence_after_sync();
@@ -109,11 +112,14 @@ k_layer_bf16(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ 
             }
         }
     } else if (warp == 1) {
-        // ===================================================== MMA issuer
-        if (lane == 0) {
+        // ===================================================== MMA issuer (whole warp; one elected lane issues)
+        // warp-uniform control flow + one elect.sync branch per k-block lets ptxas keep the descriptors in uniform
+        // registers and emit the UTCHMMAs back to back (profiles/r01_fused_l1l2.md)
+        {
             int stage = 0;
             uint32_t phase = 0;
             int it = 0;
+            const uint64_t desc0 = ptx::umma_desc_sw128_kmajor(ptx::smem_u32(smem));
             for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
                 const int nt = tile % ga.tiles_n;
                 const int n_cur = min(ga.n_tile, ga.Np - nt * ga.n_tile);
@@ -126,26 +132,32 @@ k_layer_bf16(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ 
                 for (int kb = 0; kb < num_kb; ++kb) {
                     ptx::mbar_wait(&full[stage], phase);
                     ptx::tc_fence_after_sync();
-                    const uint32_t a_addr = ptx::smem_u32(sA + (size_t)stage * kABytes);
-                    const uint32_t b_addr = ptx::smem_u32(sB + (size_t)stage * kBBytesMax);
+                    const uint64_t da = desc0 + (uint64_t)(((uint32_t)stage * kABytes) >> 4);
+                    const uint64_t db = desc0 + (uint64_t)(((uint32_t)kStages * kABytes + (uint32_t)stage * kBBytesMax) >> 4);
                     const int ksteps = min(kBK / 16, (ga.Kp - kb * kBK) / 16);
-                    for (int k = 0; k < ksteps; ++k) {
-                        const uint64_t da = ptx::umma_desc_sw128_kmajor(a_addr + k * 32);
-                        const uint64_t db = ptx::umma_desc_sw128_kmajor(b_addr + k * 32);
-                        ptx::umma_bf16_ss(d_tmem, da, db, idesc, (kb | k) ? 1u : 0u);
+                    if (ptx::elect_one()) {
+                        if (ksteps == kBK / 16) {
+#pragma unroll
+                            for (int k = 0; k < kBK / 16; ++k) ptx::umma_bf16_ss(d_tmem, da + 2 * k, db + 2 * k, idesc, (kb | k) ? 1u : 0u);
+                        } else {
+                            for (int k = 0; k < ksteps; ++k) ptx::umma_bf16_ss(d_tmem, da + 2 * k, db + 2 * k, idesc, (kb | k) ? 1u : 0u);
+                        }
+                        ptx::umma_commit(&empty[stage]);  // frees the smem slot when these MMAs have read it
+                        if (kb == num_kb - 1) ptx::umma_commit(&tfull[acc]);  // accumulator complete -> epilogue
                     }
-                    ptx::umma_commit(&empty[stage]);  // frees the smem slot when these MMAs have read it
+                    __syncwarp();
                     if (++stage == kStages) {
                         stage = 0;
                         phase ^= 1;
                     }
                 }
-                ptx::umma_commit(&tfull[acc]);  // accumulator complete -> epilogue
             }
         }
     } else {
-        // ===================================================== epilogue (warps 2..5)
-        const int q = warp & 3;  // TMEM lane quarter this warp may access
+        // ===================================================== epilogue (warps 2..9)
+        // two warps per TMEM lane quarter: 32-column pieces of the accumulator alternate between them
+        const int q = warp & 3;          // TMEM lane quarter this warp may access
+        const int hsel = (warp - 2) >> 2;  // 0 / 1: which pieces
         int it = 0;
         for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
             const int mt = tile / ga.tiles_n, nt = tile % ga.tiles_n;
@@ -158,15 +170,31 @@ k_layer_bf16(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ 
             const bool row_ok = r < rows;
             const uint32_t t_addr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)acc * kMaxNT;
             const int col0 = nt * ga.n_tile;
-            for (int cc = 0; cc < n_cur; cc += 16) {
-                uint32_t v[16];
-                ptx::tmem_ld16(t_addr + cc, v);
-                ptx::tmem_ld_wait();
-                float f[16];
-                const float4 *b4 = reinterpret_cast<const float4 *>(ga.bias + col0 + cc);
+            const int n_pieces = (n_cur + 31) >> 5;
+            for (int pc = hsel; pc < n_pieces; pc += 2) {
+                const int cc = pc << 5;
+                const bool full = cc + 32 <= n_cur;  // widths are multiples of 16: a tail piece has 16 columns
+                uint32_t v[32];
+                if (full) ptx::tmem_ld32(t_addr + cc, v);
+                else {
+                    uint32_t w[16];
+                    ptx::tmem_ld16(t_addr + cc, w);
 #pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    const float4 b = __ldg(b4 + j);
+                    for (int j = 0; j < 16; ++j) v[j] = w[j];
+#pragma unroll
+                    for (int j = 16; j < 32; ++j) v[j] = 0u;
+                }
+                ptx::tmem_ld_wait();
+                if (pc + 2 >= n_pieces) {  // last accumulator read of this warp
+                    ptx::tc_fence_before_sync();
+                    __syncwarp();
+                    if (lane == 0) ptx::mbar_arrive(&tempty[acc]);
+                }
+                float f[32];
+                const float4 *b4 = reinterpret_cast<const float4 *>(sBias + col0 + cc);
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    const float4 b = (full || j < 4) ? b4[j] : make_float4(0.f, 0.f, 0.f, 0.f);
                     f[4 * j + 0] = __uint_as_float(v[4 * j + 0]) + b.x;
                     f[4 * j + 1] = __uint_as_float(v[4 * j + 1]) + b.y;
                     f[4 * j + 2] = __uint_as_float(v[4 * j + 2]) + b.z;
@@ -174,34 +202,30 @@ k_layer_bf16(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ 
                 }
                 if (ga.apply_gelu) {
 #pragma unroll
-                    for (int j = 0; j < 16; ++j) f[j] = gelu_tanh(f[j]);
+                    for (int j = 0; j < 32; ++j) f[j] = gelu_tanh(f[j]);
                 }
                 if (ga.out_bf16) {
                     if (row_ok) {
-                        uint4 o0, o1;
-                        o0.x = ptx::pack_bf16x2(f[0], f[1]);
-                        o0.y = ptx::pack_bf16x2(f[2], f[3]);
-                        o0.z = ptx::pack_bf16x2(f[4], f[5]);
-                        o0.w = ptx::pack_bf16x2(f[6], f[7]);
-                        o1.x = ptx::pack_bf16x2(f[8], f[9]);
-                        o1.y = ptx::pack_bf16x2(f[10], f[11]);
-                        o1.z = ptx::pack_bf16x2(f[12], f[13]);
-                        o1.w = ptx::pack_bf16x2(f[14], f[15]);
                         uint4 *dst = reinterpret_cast<uint4 *>(ga.out_bf16 + r * ga.out_ld + col0 + cc);
-                        dst[0] = o0;
-                        dst[1] = o1;
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) {
+                            if (full || j < 2)
+                                dst[j] = make_uint4(ptx::pack_bf16x2(f[8 * j], f[8 * j + 1]), ptx::pack_bf16x2(f[8 * j + 2], f[8 * j + 3]),
+                                                    ptx::pack_bf16x2(f[8 * j + 4], f[8 * j + 5]), ptx::pack_bf16x2(f[8 * j + 6], f[8 * j + 7]));
+                        }
                     }
                 } else if (row_ok) {
 #pragma unroll
-                    for (int j = 0; j < 16; ++j) {
+                    for (int j = 0; j < 32; ++j) {
                         const int col = col0 + cc + j;
                         if (col < ga.N) ga.out_f32[(int64_t)col * ga.out_f32_stride + r] = f[j];
                     }
                 }
             }
-            ptx::tc_fence_before_sync();
-            __syncwarp();
-            if (lane == 0) ptx::mbar_arrive(&tempty[acc]);
+            if (hsel >= n_pieces) {  // this warp had no piece in this tile: still release the accumulator
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive(&tempty[acc]);
+            }
         }
     }
 

@@ -161,14 +161,26 @@ cudaError_t launch_pre_bf16(Ctx *c, int64_t n, int64_t c0, int64_t cn, const flo
 }
 
 // ================================================================ S4-S7 as a stand-alone kernel
-// One thread per cell of the chunk.  o[k*o_stride + i] is the raw network output of local cell i.
-// Writes Y_new (FP32, in place) and T_new; skipped / out-of-range cells are not touched.
-__global__ void __launch_bounds__(128) k_post(int64_t n, int64_t c0, int64_t cn, float *__restrict__ T,
-                                              float *__restrict__ Y, const float *__restrict__ h,
-                                              const float *__restrict__ o, int64_t o_stride, double dt,
-                                              const int32_t *__restrict__ idx, const int32_t *__restrict__ n_active,
-                                              const ThermoDev *__restrict__ thermo_g, Counters *__restrict__ counters,
-                                              float lambda_f, const PostParams pp) {
+// FOUR lanes per cell (a "quad"): lane s of the quad owns the species k = s, s + 4, s + 8, ...; the sums over the
+// species (renormalisation, Newton residual and slope) are xor-butterfly reductions inside the quad, which give all
+// four lanes bit-identical results, so they take the same Newton decisions.  Per-thread state is NSL = ceil(Ns/4)
+// doubles: registers, high occupancy.  (One thread per cell with run-time indexed double[64] arrays kept them in
+// local memory: 0.47 ms per 1 M cells; fully unrolled over 21 species it needed 128-160 registers: 0.52 ms.)
+// o[k*o_stride + i] is the raw network output of local cell i.  Writes Y_new (FP32, in place) and T_new; skipped /
+// out-of-range cells are not touched.
+__device__ __forceinline__ double quad_sum(double x) {
+    x += __shfl_xor_sync(0xffffffffu, x, 1);
+    x += __shfl_xor_sync(0xffffffffu, x, 2);
+    return x;
+}
+
+template <int NSL>
+__global__ void __launch_bounds__(128) k_post_q(int64_t n, int64_t c0, int64_t cn, float *__restrict__ T,
+                                                float *__restrict__ Y, const float *__restrict__ h,
+                                                const float *__restrict__ o, int64_t o_stride, double dt,
+                                                const int32_t *__restrict__ idx, const int32_t *__restrict__ n_active,
+                                                const ThermoDev *__restrict__ thermo_g, Counters *__restrict__ counters,
+                                                float lambda_f, const PostParams pp) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     ThermoDev *th = reinterpret_cast<ThermoDev *>(smem_raw);
     {
@@ -178,7 +190,9 @@ __global__ void __launch_bounds__(128) k_post(int64_t n, int64_t c0, int64_t cn,
         for (int w = threadIdx.x; w < words; w += blockDim.x) dst[w] = src[w];
     }
     __syncthreads();
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t i = t >> 2;     // local cell of this quad
+    const int s = (int)(t & 3);   // species slice
     const int Ns = pp.n_species;
     bool valid = i < cn;
     int64_t g = c0 + i;
@@ -186,23 +200,81 @@ __global__ void __launch_bounds__(128) k_post(int64_t n, int64_t c0, int64_t cn,
         valid = g < (int64_t)*n_active;
         g = valid ? (int64_t)idx[g] : 0;
     }
-    unsigned nconv = 0, ndeg = 0;
-    if (valid) {
-        double Yc[kMaxSpecies], Ys[kMaxSpecies];
-#pragma unroll 1
-        for (int k = 0; k < Ns; ++k) {
-            const float yf = fmaxf(Y[(int64_t)k * n + g], 0.f);
-            const float u = boxcox_u(yf, lambda_f);
-            Yc[k] = (double)yf;
-            Ys[k] = update_species((double)yf, u, o[(int64_t)k * o_stride + i], pp.out_std[k], pp.out_mean[k], dt, pp);
+    if (!valid) g = 0;
+    // invalid quads run along on zeros (the shuffles need every lane) and store nothing
+    float yin[NSL], oin[NSL];
+#pragma unroll
+    for (int j = 0; j < NSL; ++j) {  // loads first: 2 NSL independent requests in flight
+        const int k = s + 4 * j;
+        const bool on = valid && k < Ns;
+        yin[j] = on ? Y[(int64_t)k * n + g] : 0.f;
+        oin[j] = on ? o[(int64_t)k * o_stride + i] : 0.f;
+    }
+    const double hc = valid ? (double)h[g] : 0.0, T0 = valid ? (double)T[g] : 300.0;
+    double Ys[NSL];
+    double S = 0.0, Sc = 0.0;
+#pragma unroll
+    for (int j = 0; j < NSL; ++j) {
+        const int k = s + 4 * j;
+        const float yf = fmaxf(yin[j], 0.f);
+        Ys[j] = (k < Ns) ? update_species((double)yf, boxcox_u(yf, lambda_f), oin[j], pp.out_std[k < Ns ? k : 0],
+                                          pp.out_mean[k < Ns ? k : 0], dt, pp)
+                         : 0.0;
+        S += Ys[j];
+        Sc += (double)yf;
+    }
+    S = quad_sum(S);
+    Sc = quad_sum(Sc);  // (outside the branch below: the shuffles are warp-wide)
+    unsigned ndeg = 0, nconv = 0;
+    if (S > 0.0) {
+#pragma unroll
+        for (int j = 0; j < NSL; ++j) Ys[j] = Ys[j] / S;
+    } else {  // R8: vanishing sum -> max(Y,0)/sum, counted once per cell
+        ndeg = (valid && s == 0) ? 1u : 0u;
+#pragma unroll
+        for (int j = 0; j < NSL; ++j) Ys[j] = (double)fmaxf(yin[j], 0.f) / Sc;
+    }
+    // S7: Newton on the pre-scaled NASA-7 table (the arithmetic of post.cuh newton_T, species split over the quad)
+    double Tn = fmin(fmax(T0, pp.T_min), pp.T_max);
+    bool conv = false, done = false;
+    const int two = th->two_ranges;
+    for (int it = 0; it < pp.newton_max_iter; ++it) {
+        double f = 0.0, c = 0.0;
+#pragma unroll
+        for (int j = 0; j < NSL; ++j) {
+            const int k = s + 4 * j;
+            if (k < Ns) {
+                const int r = (two && !(Tn < th->T_mid[k])) ? 1 : 0;
+                const double *cp = th->cp[k][r];
+                const double *hh = th->hh[k][r];
+                const double cpk = cp[0] + Tn * (cp[1] + Tn * (cp[2] + Tn * (cp[3] + Tn * cp[4])));
+                const double hk = hh[0] + Tn * (hh[1] + Tn * (hh[2] + Tn * (hh[3] + Tn * (hh[4] + Tn * hh[5]))));
+                f = fma(Ys[j], hk, f);
+                c = fma(Ys[j], cpk, c);
+            }
         }
-        if (renormalise<kMaxSpecies>(Ys, Yc, Ns)) ndeg = 1;
-        bool conv;
-        const double Tn = newton_T<kMaxSpecies>(Ys, Ns, (double)h[g], (double)T[g], th, pp, &conv);
-        if (!conv) nconv = 1;
-#pragma unroll 1
-        for (int k = 0; k < Ns; ++k) Y[(int64_t)k * n + g] = (float)Ys[k];
-        T[g] = (float)Tn;
+        // warp-wide shuffles: quads that have finished keep computing on their frozen state
+        f = quad_sum(f) - hc;
+        c = quad_sum(c);
+        if (!done) {
+            if (!(c > 0.0)) {
+                done = true;  // R10: stop, not converged
+            } else {
+                const double dT = -f / c;
+                Tn = fmin(fmax(Tn + dT, pp.T_min), pp.T_max);
+                if (fabs(dT) < pp.newton_tol) conv = done = true;
+            }
+        }
+        if (__all_sync(0xffffffffu, done)) break;
+    }
+    if (valid) {
+        if (!conv && s == 0) nconv = 1u;
+#pragma unroll
+        for (int j = 0; j < NSL; ++j) {
+            const int k = s + 4 * j;
+            if (k < Ns) Y[(int64_t)k * n + g] = (float)Ys[j];
+        }
+        if (s == 0) T[g] = (float)Tn;
     }
     // statistics: one atomic per warp and counter, only when something happened
     nconv = __reduce_add_sync(0xffffffffu, nconv);
@@ -213,14 +285,23 @@ __global__ void __launch_bounds__(128) k_post(int64_t n, int64_t c0, int64_t cn,
     }
 }
 
+template <int NSL>
+static void launch_post_q(Ctx *c, int64_t n, int64_t c0, int64_t cn, float *T, float *Y, const float *h, const float *o,
+                          int64_t o_stride, double dt, const int32_t *ix, cudaStream_t s) {
+    const unsigned blocks = (unsigned)((cn * 4 + 127) / 128);
+    k_post_q<NSL><<<blocks, 128, sizeof(ThermoDev), s>>>(n, c0, cn, T, Y, h, o, o_stride, dt, ix, c->n_active_dev,
+                                                         c->thermo_dev, c->counters, (float)c->lambda, c->post);
+}
+
 cudaError_t launch_post(Ctx *c, int64_t n, int64_t c0, int64_t cn, float *T, float *Y, const float *h, const float *o,
                         int64_t o_stride, double dt, bool use_idx, cudaStream_t s) {
     if (cn <= 0) return cudaSuccess;
-    const int blocks = (int)((cn + 127) / 128);
     LaunchScope ls(c, kClsPost, s);
-    k_post<<<blocks, 128, sizeof(ThermoDev), s>>>(n, c0, cn, T, Y, h, o, o_stride, dt, use_idx ? c->idx : nullptr,
-                                                   c->n_active_dev, c->thermo_dev, c->counters, (float)c->lambda,
-                                                   c->post);
+    const int32_t *ix = use_idx ? c->idx : nullptr;
+    if (c->Ns <= 12) launch_post_q<3>(c, n, c0, cn, T, Y, h, o, o_stride, dt, ix, s);
+    else if (c->Ns <= 24) launch_post_q<6>(c, n, c0, cn, T, Y, h, o, o_stride, dt, ix, s);
+    else if (c->Ns <= 40) launch_post_q<10>(c, n, c0, cn, T, Y, h, o, o_stride, dt, ix, s);
+    else launch_post_q<16>(c, n, c0, cn, T, Y, h, o, o_stride, dt, ix, s);
     return cudaGetLastError();
 }
 

@@ -277,8 +277,10 @@ int gpuann_load_net(gpuann_ctx *c, int n_species, int n_layers, const int *sizes
         mac += (int64_t)ly.Kp * ly.Np;
         std::vector<uint16_t> hw((size_t)ly.Np * ly.Kp, 0);
         std::vector<float> hb((size_t)ly.Np, 0.f);
+        // every hidden activation is stored as 2 GELU(.) (ptx::gelu2_pack): its consumer W_l, l >= 1, carries the 1/2
+        const float wscale = l >= 1 ? 0.5f : 1.f;
         for (int j = 0; j < ly.N; ++j) {
-            for (int i = 0; i < ly.K; ++i) hw[(size_t)j * ly.Kp + i] = f32_to_bf16_rne(weights[l][(size_t)j * ly.K + i]);
+            for (int i = 0; i < ly.K; ++i) hw[(size_t)j * ly.Kp + i] = f32_to_bf16_rne(wscale * weights[l][(size_t)j * ly.K + i]);
             hb[j] = biases[l][j];
         }
         CU_TRY(c, cudaMalloc(&ly.W, hw.size() * sizeof(uint16_t)), "cudaMalloc(W bf16)");

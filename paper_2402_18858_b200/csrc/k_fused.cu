@@ -73,12 +73,6 @@ struct FusedArgs {
     PreParams pre;
 };
 
-__device__ __forceinline__ float gelu_tanh_f(float v) {
-    const float u = v * (0.7978845608028654f + 0.0356774081363001f * v * v);
-    const float hv = 0.5f * v;
-    return fmaf(hv, ptx::tanh_approx(u), hv);
-}
-
 // ring position: stage index + phase bit, advanced without integer division
 struct Ring {
     uint32_t st = 0, ph = 0;
@@ -340,7 +334,7 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
             uint32_t o[16];
 #pragma unroll
             for (int j = 0; j < 16; ++j)
-                o[j] = ptx::pack_bf16x2(gelu_tanh_f(__uint_as_float(v[2 * j])), gelu_tanh_f(__uint_as_float(v[2 * j + 1])));
+                o[j] = ptx::gelu2_pack(__uint_as_float(v[2 * j]), __uint_as_float(v[2 * j + 1]));
             ptx::mbar_wait(&bars[bAEmpty + a.st], a.ph ^ 1u);
             const uint32_t row_addr = sbase + kOffA + a.st * kAStageBytes + row_off;
 #pragma unroll
@@ -400,10 +394,8 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
 #pragma unroll
                     for (int j = 0; j < 8; ++j) {
                         const float4 b = (full || j < 4) ? b4[j] : make_float4(0.f, 0.f, 0.f, 0.f);
-                        o[2 * j] = ptx::pack_bf16x2(gelu_tanh_f(__uint_as_float(v[4 * j]) + b.x),
-                                                    gelu_tanh_f(__uint_as_float(v[4 * j + 1]) + b.y));
-                        o[2 * j + 1] = ptx::pack_bf16x2(gelu_tanh_f(__uint_as_float(v[4 * j + 2]) + b.z),
-                                                        gelu_tanh_f(__uint_as_float(v[4 * j + 3]) + b.w));
+                        o[2 * j] = ptx::gelu2_pack(__uint_as_float(v[4 * j]) + b.x, __uint_as_float(v[4 * j + 1]) + b.y);
+                        o[2 * j + 1] = ptx::gelu2_pack(__uint_as_float(v[4 * j + 2]) + b.z, __uint_as_float(v[4 * j + 3]) + b.w);
                     }
                     if (row_ok) {
                         uint4 *dst = reinterpret_cast<uint4 *>(dst_row + cc);

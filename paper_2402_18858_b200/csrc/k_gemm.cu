@@ -200,18 +200,23 @@ k_layer_bf16(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ 
                     f[4 * j + 2] = __uint_as_float(v[4 * j + 2]) + b.z;
                     f[4 * j + 3] = __uint_as_float(v[4 * j + 3]) + b.w;
                 }
-                if (ga.apply_gelu) {
-#pragma unroll
-                    for (int j = 0; j < 32; ++j) f[j] = gelu_tanh(f[j]);
-                }
                 if (ga.out_bf16) {
+                    // hidden layer: 2 GELU(.) packed to BF16 (the 1/2 is in the next layer's weights, api.cu)
                     if (row_ok) {
                         uint4 *dst = reinterpret_cast<uint4 *>(ga.out_bf16 + r * ga.out_ld + col0 + cc);
 #pragma unroll
                         for (int j = 0; j < 4; ++j) {
-                            if (full || j < 2)
-                                dst[j] = make_uint4(ptx::pack_bf16x2(f[8 * j], f[8 * j + 1]), ptx::pack_bf16x2(f[8 * j + 2], f[8 * j + 3]),
-                                                    ptx::pack_bf16x2(f[8 * j + 4], f[8 * j + 5]), ptx::pack_bf16x2(f[8 * j + 6], f[8 * j + 7]));
+                            if (full || j < 2) {
+                                uint4 o;
+                                if (ga.apply_gelu) {
+                                    o = make_uint4(ptx::gelu2_pack(f[8 * j], f[8 * j + 1]), ptx::gelu2_pack(f[8 * j + 2], f[8 * j + 3]),
+                                                   ptx::gelu2_pack(f[8 * j + 4], f[8 * j + 5]), ptx::gelu2_pack(f[8 * j + 6], f[8 * j + 7]));
+                                } else {
+                                    o = make_uint4(ptx::pack_bf16x2(f[8 * j], f[8 * j + 1]), ptx::pack_bf16x2(f[8 * j + 2], f[8 * j + 3]),
+                                                   ptx::pack_bf16x2(f[8 * j + 4], f[8 * j + 5]), ptx::pack_bf16x2(f[8 * j + 6], f[8 * j + 7]));
+                                }
+                                dst[j] = o;
+                            }
                         }
                     }
                 } else if (row_ok) {

@@ -279,5 +279,32 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
     return r;
 }
 
+// Two activations at once, packed to BF16x2: returns 2 GELU(v) = v + v tanh(u), u = v (c0 + c1 v^2) (tanh form, R5).
+// The factor 1/2 lives in the NEXT layer's weights (exact in BF16; api.cu scales W_l, l >= 2, of the tensor path), and
+// the polynomial runs on packed FP32x2 instructions (mul/fma.f32x2): 7 instructions per pair instead of 15.
+__device__ __forceinline__ uint32_t gelu2_pack(float v0, float v1) {
+    uint32_t out;
+    asm("{\n\t"
+        ".reg .b64 x, w, t, c0, c1;\n\t"
+        ".reg .f32 a, b;\n\t"
+        "mov.b64 x, {%1, %2};\n\t"
+        "mov.b64 c0, {%3, %3};\n\t"
+        "mov.b64 c1, {%4, %4};\n\t"
+        "mul.f32x2 w, x, x;\n\t"
+        "fma.rn.f32x2 t, w, c1, c0;\n\t"
+        "mul.f32x2 t, x, t;\n\t"
+        "mov.b64 {a, b}, t;\n\t"
+        "tanh.approx.f32 a, a;\n\t"
+        "tanh.approx.f32 b, b;\n\t"
+        "mov.b64 t, {a, b};\n\t"
+        "fma.rn.f32x2 t, x, t, x;\n\t"
+        "mov.b64 {a, b}, t;\n\t"
+        "cvt.rn.bf16x2.f32 %0, b, a;\n\t"
+        "}\n"
+        : "=r"(out)
+        : "f"(v0), "f"(v1), "f"(0.7978845608028654f), "f"(0.0356774081363001f));
+    return out;
+}
+
 }  // namespace ptx
 }  // namespace gpuann

@@ -270,9 +270,10 @@ int gpuann_load_net(gpuann_ctx *c, int n_species, int n_layers, const int *sizes
         ly.N = sizes[l + 1];
         ly.Kp = pad16(ly.K);
         ly.Np = pad16(ly.N);
-        ly.tiles_n = (ly.Np + 255) / 256;
+        ly.tiles_n = (ly.Np + 415) / 416;
         ly.n_tile = pad16((ly.Np + ly.tiles_n - 1) / ly.tiles_n);
         ly.tiles_n = (ly.Np + ly.n_tile - 1) / ly.n_tile;
+        ly.n0 = ly.n_tile > 256 ? pad16((ly.n_tile + 1) / 2) : 0;
         if (!fused || l >= 2) maxKp = ly.Kp > maxKp ? ly.Kp : maxKp;
         mac += (int64_t)ly.Kp * ly.Np;
         std::vector<uint16_t> hw((size_t)ly.Np * ly.Kp, 0);
@@ -288,7 +289,7 @@ int gpuann_load_net(gpuann_ctx *c, int n_species, int n_layers, const int *sizes
         CU_TRY(c, cudaMemcpy(ly.W, hw.data(), hw.size() * sizeof(uint16_t), cudaMemcpyHostToDevice), "cudaMemcpy(W)");
         CU_TRY(c, cudaMemcpy(ly.bias, hb.data(), hb.size() * sizeof(float), cudaMemcpyHostToDevice), "cudaMemcpy(bias)");
         std::string terr;
-        if (!encode_tmap_bf16(&ly.tmapW, ly.W, (uint64_t)ly.Kp, (uint64_t)ly.Np, (uint64_t)ly.Kp * 2, (uint32_t)ly.n_tile, &terr))
+        if (!encode_tmap_bf16(&ly.tmapW, ly.W, (uint64_t)ly.Kp, (uint64_t)ly.Np, (uint64_t)ly.Kp * 2, (uint32_t)(ly.n0 > 0 ? ly.n0 : ly.n_tile), &terr))
             return fail(c, GPUANN_ERR_CUDA, "gpuann_load_net: " + terr);
     }
     if (fused) {

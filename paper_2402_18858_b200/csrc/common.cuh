@@ -64,7 +64,8 @@ struct Counters {
 struct LayerBf16 {
     int K, N;            // true fan-in / fan-out
     int Kp, Np;          // padded to multiples of 16
-    int n_tile;          // UMMA N of a full tile (multiple of 16, <= 256)
+    int n_tile;          // columns of a full tile (multiple of 16, <= 416)
+    int n0;              // n_tile > 256: columns of the first of the two MMAs per k-step (= TMA box rows); else 0
     int tiles_n;         // ceil(Np / n_tile)
     __nv_bfloat16 *W;    // DEVICE [Np][Kp] row-major, zero padded
     float *bias;         // DEVICE [Np], zero padded

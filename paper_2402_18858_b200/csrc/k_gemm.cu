@@ -21,7 +21,14 @@ constexpr int kGemmThreads = 320;   // TMA, MMA, 8 epilogue warps
 constexpr uint32_t kABytes = kBM * kBK * 2;        // 16 KB
 constexpr uint32_t kBBytesMax = kMaxNT * kBK * 2;  // 32 KB
 constexpr int kBiasMax = 4096;  // = GPUANN_MAX_WIDTH floats staged in shared memory
-constexpr size_t kGemmSmem = 1024 /*align slack*/ + (size_t)kStages * (kABytes + kBBytesMax) + 256 + kBiasMax * 4;
+// "wide" tiles (n_tile > 256: two MMAs per k-step into ONE accumulator of up to 416 columns, A read once for the
+// whole row of W): 3 stages of A 16 KB + B 52 KB; narrow tiles: 4 stages of 16 + 32 KB and two accumulators
+constexpr int kWideStages = 3;
+constexpr uint32_t kBBytesWide = 416 * kBK * 2;  // 53,248
+constexpr size_t kRegion = (size_t)kWideStages * (kABytes + kBBytesWide) > (size_t)kStages * (kABytes + kBBytesMax)
+                               ? (size_t)kWideStages * (kABytes + kBBytesWide)
+                               : (size_t)kStages * (kABytes + kBBytesMax);
+constexpr size_t kGemmSmem = 1024 /*align slack*/ + kRegion + 256 + kBiasMax * 4;
 
 // GELU in the tanh form, tanh.approx.f32 (R5: any evaluation inside the BF16 tolerances)
 __device__ __forceinline__ float gelu_tanh(float v) {
@@ -33,6 +40,7 @@ __device__ __forceinline__ float gelu_tanh(float v) {
 struct GemmArgs {
     int Kp, Np, N;          // padded K, padded N, true N
     int n_tile, tiles_n;
+    int n0;                 // wide tiles (n_tile > 256): columns of the first MMA (= TMA box rows); 0 = narrow
     int64_t rows;           // valid rows when n_active == nullptr
     int64_t c0;             // first (compacted) cell of this chunk, for the n_active test
     const int32_t *n_active;  // DEVICE or nullptr: rows = clamp(*n_active - c0, 0, rows)
@@ -49,11 +57,14 @@ k_layer_bf16(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ 
     extern __shared__ unsigned char smem_raw[];
     unsigned char *smem = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     unsigned char *sA = smem;
-    unsigned char *sB = smem + (size_t)kStages * kABytes;
-    uint64_t *bars = reinterpret_cast<uint64_t *>(sB + (size_t)kStages * kBBytesMax);
+    const bool wide = ga.n0 > 0;
+    const int nst = wide ? kWideStages : kStages;
+    const uint32_t bsz = wide ? kBBytesWide : kBBytesMax;
+    unsigned char *sB = smem + (size_t)nst * kABytes;
+    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + kRegion);
     uint64_t *full = bars, *empty = bars + kStages, *tfull = bars + 2 * kStages, *tempty = bars + 2 * kStages + 2;
     uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(bars + 2 * kStages + 4);
-    float *sBias = reinterpret_cast<float *>(sB + (size_t)kStages * kBBytesMax + 256);
+    float *sBias = reinterpret_cast<float *>(smem + kRegion + 256);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -65,7 +76,7 @@ k_layer_bf16(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ 
     const int tiles_m = (int)((rows + kBM - 1) / kBM);
     const int n_tiles = tiles_m * ga.tiles_n;
     const int num_kb = (ga.Kp + kBK - 1) / kBK;
-    const uint32_t b_bytes = (uint32_t)ga.n_tile * kBK * 2;
+    const uint32_t b_bytes = (wide ? 2u * (uint32_t)ga.n0 : (uint32_t)ga.n_tile) * kBK * 2;
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < kStages; ++s) {
@@ -103,8 +114,11 @@ k_layer_bf16(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ 
                     ptx::mbar_wait(&empty[stage], phase ^ 1);
                     ptx::mbar_arrive_expect_tx(&full[stage], kABytes + b_bytes);
                     ptx::tma_load_2d(&tmapA, &full[stage], sA + (size_t)stage * kABytes, kb * kBK, mt * kBM);
-                    ptx::tma_load_2d(&tmapW, &full[stage], sB + (size_t)stage * kBBytesMax, kb * kBK, nt * ga.n_tile);
-                    if (++stage == kStages) {
+                    ptx::tma_load_2d(&tmapW, &full[stage], sB + (size_t)stage * bsz, kb * kBK, nt * ga.n_tile);
+                    if (wide)  // second box: rows n0.. (rows beyond Np are zero filled)
+                        ptx::tma_load_2d(&tmapW, &full[stage], sB + (size_t)stage * bsz + (size_t)ga.n0 * 128, kb * kBK,
+                                         nt * ga.n_tile + ga.n0);
+                    if (++stage == nst) {
                         stage = 0;
                         phase ^= 1;
                     }
@@ -123,9 +137,12 @@ k_layer_bf16(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ 
             for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
                 const int nt = tile % ga.tiles_n;
                 const int n_cur = min(ga.n_tile, ga.Np - nt * ga.n_tile);
-                const uint32_t idesc = ptx::umma_idesc_bf16_f32(kBM, (uint32_t)n_cur);
-                const int acc = it & 1;
-                const uint32_t acc_phase = (uint32_t)(it >> 1) & 1;
+                const int n0_cur = wide ? min(ga.n0, n_cur) : n_cur, n1_cur = n_cur - n0_cur;
+                const uint32_t idesc = ptx::umma_idesc_bf16_f32(kBM, (uint32_t)n0_cur);
+                const uint32_t idesc1 = ptx::umma_idesc_bf16_f32(kBM, (uint32_t)(n1_cur > 0 ? n1_cur : 16));
+                const uint64_t b1_off = (uint64_t)(((uint32_t)ga.n0 * 128u) >> 4);
+                const int acc = wide ? 0 : (it & 1);
+                const uint32_t acc_phase = wide ? ((uint32_t)it & 1) : ((uint32_t)(it >> 1) & 1);
                 ptx::mbar_wait(&tempty[acc], acc_phase ^ 1);
                 ptx::tc_fence_after_sync();
                 const uint32_t d_tmem = tmem_base + (uint32_t)acc * kMaxNT;
@@ -133,20 +150,28 @@ k_layer_bf16(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ 
                     ptx::mbar_wait(&full[stage], phase);
                     ptx::tc_fence_after_sync();
                     const uint64_t da = desc0 + (uint64_t)(((uint32_t)stage * kABytes) >> 4);
-                    const uint64_t db = desc0 + (uint64_t)(((uint32_t)kStages * kABytes + (uint32_t)stage * kBBytesMax) >> 4);
+                    const uint64_t db = desc0 + (uint64_t)(((uint32_t)nst * kABytes + (uint32_t)stage * bsz) >> 4);
                     const int ksteps = min(kBK / 16, (ga.Kp - kb * kBK) / 16);
                     if (ptx::elect_one()) {
                         if (ksteps == kBK / 16) {
 #pragma unroll
-                            for (int k = 0; k < kBK / 16; ++k) ptx::umma_bf16_ss(d_tmem, da + 2 * k, db + 2 * k, idesc, (kb | k) ? 1u : 0u);
+                            for (int k = 0; k < kBK / 16; ++k) {
+                                ptx::umma_bf16_ss(d_tmem, da + 2 * k, db + 2 * k, idesc, (kb | k) ? 1u : 0u);
+                                if (n1_cur > 0)
+                                    ptx::umma_bf16_ss(d_tmem + (uint32_t)ga.n0, da + 2 * k, db + b1_off + 2 * k, idesc1, (kb | k) ? 1u : 0u);
+                            }
                         } else {
-                            for (int k = 0; k < ksteps; ++k) ptx::umma_bf16_ss(d_tmem, da + 2 * k, db + 2 * k, idesc, (kb | k) ? 1u : 0u);
+                            for (int k = 0; k < ksteps; ++k) {
+                                ptx::umma_bf16_ss(d_tmem, da + 2 * k, db + 2 * k, idesc, (kb | k) ? 1u : 0u);
+                                if (n1_cur > 0)
+                                    ptx::umma_bf16_ss(d_tmem + (uint32_t)ga.n0, da + 2 * k, db + b1_off + 2 * k, idesc1, (kb | k) ? 1u : 0u);
+                            }
                         }
                         ptx::umma_commit(&empty[stage]);  // frees the smem slot when these MMAs have read it
                         if (kb == num_kb - 1) ptx::umma_commit(&tfull[acc]);  // accumulator complete -> epilogue
                     }
                     __syncwarp();
-                    if (++stage == kStages) {
+                    if (++stage == nst) {
                         stage = 0;
                         phase ^= 1;
                     }
@@ -162,8 +187,8 @@ k_layer_bf16(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ 
         for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
             const int mt = tile / ga.tiles_n, nt = tile % ga.tiles_n;
             const int n_cur = min(ga.n_tile, ga.Np - nt * ga.n_tile);
-            const int acc = it & 1;
-            const uint32_t acc_phase = (uint32_t)(it >> 1) & 1;
+            const int acc = wide ? 0 : (it & 1);
+            const uint32_t acc_phase = wide ? ((uint32_t)it & 1) : ((uint32_t)(it >> 1) & 1);
             ptx::mbar_wait(&tfull[acc], acc_phase);
             ptx::tc_fence_after_sync();
             const int64_t r = (int64_t)mt * kBM + q * 32 + lane;
@@ -295,6 +320,7 @@ cudaError_t launch_layer_bf16(Ctx *c, int layer, int64_t rows, const CUtensorMap
     ga.N = ly.N;
     ga.n_tile = ly.n_tile;
     ga.tiles_n = ly.tiles_n;
+    ga.n0 = ly.n0;
     ga.rows = rows;
     ga.c0 = c0;
     ga.n_active = use_count ? c->n_active_dev : nullptr;

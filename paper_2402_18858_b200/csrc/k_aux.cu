@@ -227,8 +227,9 @@ __global__ void __launch_bounds__(128) k_post_q(int64_t n, int64_t c0, int64_t c
     Sc = quad_sum(Sc);  // (outside the branch below: the shuffles are warp-wide)
     unsigned ndeg = 0, nconv = 0;
     if (S > 0.0) {
+        const double rS = 1.0 / S;  // one division per thread; Y* rS differs from Y*/S by <= 1 ulp of FP64
 #pragma unroll
-        for (int j = 0; j < NSL; ++j) Ys[j] = Ys[j] / S;
+        for (int j = 0; j < NSL; ++j) Ys[j] = Ys[j] * rS;
     } else {  // R8: vanishing sum -> max(Y,0)/sum, counted once per cell
         ndeg = (valid && s == 0) ? 1u : 0u;
 #pragma unroll

@@ -259,7 +259,7 @@ int gpuann_load_net(gpuann_ctx *c, int n_species, int n_layers, const int *sizes
     const char *force = std::getenv("GPUANN_VARIANT");
     const bool want_fused = !(force && std::strcmp(force, "layerwise") == 0);
     const bool fused = want_fused && n_layers >= 3 && fused_supported(sizes[0], sizes[1], pad16(sizes[2]));
-    int64_t chunk = c->prm.chunk_cells > 0 ? c->prm.chunk_cells : (int64_t)c->sm_count * 128 * (fused ? 16 : 1);
+    int64_t chunk = c->prm.chunk_cells > 0 ? c->prm.chunk_cells : (int64_t)c->sm_count * 128 * (fused ? 56 : 1);
     chunk = (chunk + 127) / 128 * 128;
     c->chunk = chunk;
     int maxKp = 0;

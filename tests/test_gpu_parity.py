@@ -95,3 +95,83 @@ def test_c4_compaction_reduced_n():
         print(f"c4 n={n}: active {int(active.sum())}, dT {dT:.3e} K")
     finally:
         B.gpuann_destroy(ctx)
+
+
+def _sample_indices(n, rng, extra):
+    """First 4,096, last 4,096 and `extra` seed-drawn cells: tiles at both ends + scattered ones."""
+    head = np.arange(0, min(4096, n))
+    tail = np.arange(max(0, n - 4096), n)
+    mid = rng.choice(n, size=min(extra, n), replace=False)
+    return np.unique(np.concatenate([head, tail, mid]))
+
+
+def test_c2_full_size_sampled_and_invariants():
+    """configs[2] at its FULL size (1,048,576 cells) in the launch configuration bench.py times (default chunk):
+    full-field invariants on every cell, oracle parity on a sample the oracle computes cell by cell."""
+    cfg = I.get_config("c2")
+    pr = G.prepare(cfg)
+    n = cfg.n_cells
+    ctx = G.make_ctx(pr)
+    try:
+        g = G.run_gpu(ctx, pr)
+        assert g.stats[0] == n and g.stats[1] == 0 and g.stats[2] == 0
+        assert np.isfinite(g.T_new).all() and np.isfinite(g.Y_new).all() and np.isfinite(g.o_raw).all()
+        assert (g.T_new >= cfg.T_min).all() and (g.T_new <= cfg.T_max).all()
+        assert (g.Y_new >= 0).all()
+        G.check_sumY(g.Y_new)
+        idx = _sample_indices(n, np.random.default_rng(20260218), 8192)
+        st = pr.prob.state
+        ref = G.run_oracle(pr, T=st.T[idx], p=st.p[idx], Y=np.ascontiguousarray(st.Y[:, idx]), h=pr.h[idx])
+        sub = G.GpuResult(g.T_new[idx], np.ascontiguousarray(g.Y_new[:, idx]), np.ascontiguousarray(g.o_raw[:, idx]), g.stats)
+        l2, mx = G.check_raw_bf16(sub.o_raw, ref.o_raw)
+        dT = G.check_T_bf16(sub, ref)
+        print(f"c2 full: {idx.size} sampled cells, raw rel-L2 {l2:.2e}, max/colmax {mx:.2e}, dT {dT:.3e} K")
+    finally:
+        B.gpuann_destroy(ctx)
+
+
+def test_bf16_step_is_deterministic_and_cellwise():
+    """Two runs are bit-identical, and a cell's result does not depend on the batch it sits in (permutation)."""
+    n = 128 * 6 + 11
+    pr = G.prepare(I.get_config("c2"), n=n)
+    ctx = G.make_ctx(pr, chunk_cells=512)
+    try:
+        a = G.run_gpu(ctx, pr, want_raw=False)
+        b = G.run_gpu(ctx, pr, want_raw=False)
+        assert np.array_equal(a.T_new.view(np.uint32), b.T_new.view(np.uint32))
+        assert np.array_equal(a.Y_new.view(np.uint32), b.Y_new.view(np.uint32))
+        st = pr.prob.state
+        perm = np.random.default_rng(7).permutation(n)
+        c = G.run_gpu(ctx, pr, T=st.T[perm], p=st.p[perm], Y=np.ascontiguousarray(st.Y[:, perm]), h=pr.h[perm], want_raw=False)
+        assert np.array_equal(c.T_new.view(np.uint32), a.T_new[perm].view(np.uint32))
+        assert np.array_equal(c.Y_new.view(np.uint32), a.Y_new[:, perm].view(np.uint32))
+    finally:
+        B.gpuann_destroy(ctx)
+
+
+def test_abi_behaviour_on_device():
+    """n_cells = 0 is a no-op, chem_step before the loads is NOT_READY, bad arguments are INVALID_ARG (no abort)."""
+    import torch
+    prm = B.gpuann_default_params()
+    ctx = B.gpuann_create(prm)
+    try:
+        t = torch.zeros(8, dtype=torch.float32, device="cuda:0")
+        y = torch.zeros(21 * 8, dtype=torch.float32, device="cuda:0")
+        with pytest.raises(B.GpuannError) as e:
+            B.gpuann_chem_step(ctx, 8, t.data_ptr(), t.data_ptr(), y.data_ptr(), t.data_ptr(), 1e-6, 0)
+        assert e.value.status == B.GPUANN_ERR_NOT_READY
+    finally:
+        B.gpuann_destroy(ctx)
+    pr = G.prepare(I.get_config("c0"), n=64)
+    ctx = G.make_ctx(pr)
+    try:
+        t = torch.zeros(64, dtype=torch.float32, device="cuda:0")
+        y = torch.zeros(9 * 64, dtype=torch.float32, device="cuda:0")
+        B.gpuann_chem_step(ctx, 0, 0, 0, 0, 0, 1e-6, 0)  # n = 0: pointers are not looked at
+        for bad in (dict(n=-1), dict(dt=0.0), dict(T=0)):
+            with pytest.raises(B.GpuannError) as e:
+                B.gpuann_chem_step(ctx, bad.get("n", 64), bad.get("T", t.data_ptr()), t.data_ptr(), y.data_ptr(),
+                                   t.data_ptr(), bad.get("dt", 1e-6), 0)
+            assert e.value.status == B.GPUANN_ERR_INVALID_ARG
+    finally:
+        B.gpuann_destroy(ctx)

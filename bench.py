@@ -288,6 +288,9 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     if dom_name.startswith("layer"):
         l = int(dom_name[5])
         flop_step = 2.0 * sizes[l] * sizes[l + 1] * n_act_per_step
+    elif dom_name == "bf16_fused":
+        # the fused kernel holds layers 1 and 2 only (algorithmic: the per-pass recompute of layer 1 is not counted)
+        flop_step = 2.0 * (sizes[0] * sizes[1] + sizes[1] * sizes[2]) * n_act_per_step
     else:
         flop_step = float(cfg.flop_per_cell) * n_act_per_step
     dom_ms_per_step = dom_ms / args.steps

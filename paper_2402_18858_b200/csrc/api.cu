@@ -313,10 +313,11 @@ int gpuann_load_net(gpuann_ctx *c, int n_species, int n_layers, const int *sizes
         CU_TRY(c, cudaMemcpy(fn.W1p, w1.data(), w1.size() * sizeof(uint16_t), cudaMemcpyHostToDevice), "cudaMemcpy(W1 padded)");
         std::string terr;
         const LayerBf16 &l2 = c->lay[1];
-        if (!encode_tmap_bf16(&fn.tmapW1, fn.W1p, 64, (uint64_t)H1, 128, 64, &terr) ||
-            !encode_tmap_bf16(&fn.tmapW2a, l2.W, (uint64_t)l2.Kp, (uint64_t)l2.Np, (uint64_t)l2.Kp * 2, (uint32_t)fn.n0, &terr) ||
+        // boxes are HALF stages: each CTA of a pair loads one half and multicasts it to both (k_fused.cu)
+        if (!encode_tmap_bf16(&fn.tmapW1, fn.W1p, 64, (uint64_t)H1, 128, 32, &terr) ||
+            !encode_tmap_bf16(&fn.tmapW2a, l2.W, (uint64_t)l2.Kp, (uint64_t)l2.Np, (uint64_t)l2.Kp * 2, (uint32_t)(fn.n0 / 2), &terr) ||
             !encode_tmap_bf16(&fn.tmapW2b, l2.W, (uint64_t)l2.Kp, (uint64_t)l2.Np, (uint64_t)l2.Kp * 2,
-                              (uint32_t)(fn.n1 > 0 ? fn.n1 : 16), &terr))
+                              (uint32_t)(fn.n1 > 0 ? fn.n1 / 2 : 8), &terr))
             return fail(c, GPUANN_ERR_CUDA, "gpuann_load_net: " + terr);
         fn.on = true;
         // MACs issued: layer 1 once per pass over 16 * Kz columns, layer 2 over n_pass * pass_w columns

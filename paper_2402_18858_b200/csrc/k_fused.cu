@@ -102,12 +102,19 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
         rows = r < 0 ? 0 : (r < rows ? r : rows);
     }
     const int n_tiles = (int)((rows + kFM - 1) / kFM);
-    const int my_tiles = n_tiles > (int)blockIdx.x ? (n_tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
+    // CTAs run in clusters of two that share every weight tile: each CTA loads HALF of a W1 / W2 stage and multicasts
+    // it to both (the kernel is bound by the L2 -> SM weight stream: 2.97 MB per 128-cell tile, 8.9 TB/s measured
+    // against an L2 slice throughput cap of ~10-12 TB/s; profiles/r01_fused_l1l2.md).  Both CTAs of a pair must walk
+    // the same number of tiles; the odd one may get a tile index past the end, which it processes as an empty tile.
+    const uint32_t crank = ptx::cluster_ctarank();
+    const int pair_first = (int)blockIdx.x & ~1;
+    const int my_tiles = n_tiles > pair_first ? (n_tiles - pair_first + (int)gridDim.x - 1) / (int)gridDim.x : 0;
     const int n_chunks = fa.H1 / kFK;
 
     if (threadIdx.x == 0) {
-        for (int i = 0; i < kW2Stages; ++i) { ptx::mbar_init(&bars[bW2Full + i], 1); ptx::mbar_init(&bars[bW2Empty + i], 1); }
-        for (int i = 0; i < kW1Stages; ++i) { ptx::mbar_init(&bars[bW1Full + i], 1); ptx::mbar_init(&bars[bW1Empty + i], 1); }
+        // "empty" barriers of the weight rings collect one tcgen05.commit from EACH CTA of the pair
+        for (int i = 0; i < kW2Stages; ++i) { ptx::mbar_init(&bars[bW2Full + i], 1); ptx::mbar_init(&bars[bW2Empty + i], 2); }
+        for (int i = 0; i < kW1Stages; ++i) { ptx::mbar_init(&bars[bW1Full + i], 1); ptx::mbar_init(&bars[bW1Empty + i], 2); }
         for (int i = 0; i < kAStages; ++i) { ptx::mbar_init(&bars[bAFull + i], 8); ptx::mbar_init(&bars[bAEmpty + i], 1); }
         for (int i = 0; i < kL1Slots; ++i) { ptx::mbar_init(&bars[bL1Full + i], 1); ptx::mbar_init(&bars[bL1Empty + i], 4); }
         for (int i = 0; i < 2; ++i) { ptx::mbar_init(&bars[bZFull + i], 1); ptx::mbar_init(&bars[bZEmpty + i], 1); }
@@ -127,6 +134,7 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
     for (int i = threadIdx.x; i < fa.H2p && i < (int)(kBias2Bytes / 4); i += kFusedThreads) sBias[i] = fa.bias2[i];
     ptx::tc_fence_before_sync();
     __syncthreads();
+    ptx::cluster_sync_all();  // the peer's barriers are initialised before anything of ours can reach them
     ptx::tc_fence_after_sync();
     const uint32_t tmem_base = *tmem_slot;
 
@@ -144,7 +152,9 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
                 if (i < total) {
                     ptx::mbar_wait(&bars[bW1Empty + w1.st], w1.ph ^ 1u);
                     ptx::mbar_arrive_expect_tx(&bars[bW1Full + w1.st], kW1StageBytes);
-                    ptx::tma_load_2d(&tmapW1, &bars[bW1Full + w1.st], smem + kOffW1 + w1.st * kW1StageBytes, 0, c1 * kFK);
+                    ptx::tma_load_2d_multicast(&tmapW1, &bars[bW1Full + w1.st],
+                                               smem + kOffW1 + w1.st * kW1StageBytes + crank * (kW1StageBytes / 2), 0,
+                                               c1 * kFK + (int)crank * (kFK / 2), 3);
                     w1.next(kW1Stages);
                     if (++c1 == n_chunks) c1 = 0;
                 }
@@ -152,10 +162,13 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
                     ptx::mbar_wait(&bars[bW2Empty + w2.st], w2.ph ^ 1u);
                     ptx::mbar_arrive_expect_tx(&bars[bW2Full + w2.st], w2_bytes);
                     unsigned char *dst = smem + kOffW2 + w2.st * kW2StageBytes;
-                    ptx::tma_load_2d(&tmapW2a, &bars[bW2Full + w2.st], dst, c2 * kFK, p2 * fa.pass_w);
+                    const int h0 = fa.n0 / 2, h1 = fa.n1 / 2;  // rows of this CTA's halves of the two boxes
+                    ptx::tma_load_2d_multicast(&tmapW2a, &bars[bW2Full + w2.st], dst + (size_t)crank * h0 * 128, c2 * kFK,
+                                               p2 * fa.pass_w + (int)crank * h0, 3);
                     if (fa.n1 > 0)
-                        ptx::tma_load_2d(&tmapW2b, &bars[bW2Full + w2.st], dst + (size_t)fa.n0 * 128, c2 * kFK,
-                                         p2 * fa.pass_w + fa.n0);
+                        ptx::tma_load_2d_multicast(&tmapW2b, &bars[bW2Full + w2.st],
+                                                   dst + (size_t)fa.n0 * 128 + (size_t)crank * h1 * 128, c2 * kFK,
+                                                   p2 * fa.pass_w + fa.n0 + (int)crank * h1, 3);
                     w2.next(kW2Stages);
                     if (++c2 == n_chunks) {
                         c2 = 0;
@@ -191,7 +204,7 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
                                 ptx::umma_bf16_ss(tmem_base + (uint32_t)fa.n0, da + 2 * k, db + b1_off + 2 * k, idesc_n1, accum);
                         }
                         ptx::umma_commit(&bars[bAEmpty + a.st]);
-                        ptx::umma_commit(&bars[bW2Empty + w2.st]);
+                        ptx::umma_commit_multicast(&bars[bW2Empty + w2.st], 3);
                     }
                     __syncwarp();
                     a.next(kAStages);
@@ -229,7 +242,7 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
                         __syncwarp();
                         slot.next(kL1Slots);
                     }
-                    if (ptx::elect_one()) ptx::umma_commit(&bars[bW1Empty + w1.st]);
+                    if (ptx::elect_one()) ptx::umma_commit_multicast(&bars[bW1Empty + w1.st], 3);
                     __syncwarp();
                     w1.next(kW1Stages);
                 }
@@ -413,6 +426,7 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
 
     ptx::tc_fence_before_sync();
     __syncthreads();
+    ptx::cluster_sync_all();  // no CTA leaves while its peer may still multicast into it or signal its barriers
     if (warp == 1) {
         ptx::tc_fence_after_sync();
         ptx::tmem_dealloc(tmem_base, 512);
@@ -467,10 +481,22 @@ cudaError_t launch_fused_l1l2(Ctx *c, int64_t n, int64_t c0, int64_t cn, const f
     fa.h2 = c->act[0];
     fa.pre = c->pre;
     const int64_t tiles = (cn + kFM - 1) / kFM;
-    const int grid = (int)(tiles < c->sm_count ? tiles : c->sm_count);
+    int grid = (int)(tiles < c->sm_count ? tiles : c->sm_count);
+    grid = (grid + 1) & ~1;  // clusters of two CTAs
     LaunchScope ls(c, kClsFused, s);
-    k_fused_l1l2<<<grid, kFusedThreads, kFusedSmem, s>>>(fn.tmapW1, fn.tmapW2a, fn.tmapW2b, fa);
-    return cudaGetLastError();
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3(kFusedThreads);
+    cfg.dynamicSmemBytes = kFusedSmem;
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = 2;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, k_fused_l1l2, fn.tmapW1, fn.tmapW2a, fn.tmapW2b, fa);
 }
 
 }  // namespace gpuann

@@ -121,6 +121,34 @@ __device__ __forceinline__ uint64_t policy_evict_first() {
     return p;
 }
 
+// ---------------------------------------------------------------- thread-block clusters (pairs of CTAs)
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+// all threads of all CTAs of the cluster
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// TMA tile load delivered to the same shared-memory offset of every CTA in cta_mask; each destination CTA's
+// mbarrier at the same offset as `bar` receives the complete_tx of the bytes that landed in ITS shared memory
+__device__ __forceinline__ void tma_load_2d_multicast(const void *tmap, uint64_t *bar, void *smem_dst, int32_t c0, int32_t c1,
+                                                      uint16_t cta_mask) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster"
+        " [%0], [%1, {%3, %4}], [%2], %5;" ::"r"(smem_u32(smem_dst)),
+        "l"(reinterpret_cast<uint64_t>(tmap)), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "h"(cta_mask)
+        : "memory");
+}
+// tcgen05.commit that arrives on the mbarrier at the same offset in every CTA of cta_mask
+__device__ __forceinline__ void umma_commit_multicast(uint64_t *bar, uint16_t cta_mask) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(
+                     smem_u32(bar)),
+                 "h"(cta_mask)
+                 : "memory");
+}
+
 // ---------------------------------------------------------------- tcgen05: TMEM allocation
 // One full warp executes these (.sync.aligned).  ncols: power of two in [32, 512].
 __device__ __forceinline__ void tmem_alloc(uint32_t *smem_result, uint32_t ncols) {

@@ -447,6 +447,21 @@ int check_step_args(Ctx *c, const char *fn, int64_t n, const void *T, const void
     return GPUANN_OK;
 }
 
+struct PostArgsHost {
+    float *T, *Y;
+    const float *h;
+    double dt;
+};
+
+// one slice [a, a+len) of a device-resident field through the tensor path (no compaction): forward + update
+int step_slice_bf16(Ctx *c, int64_t n, int64_t a, int64_t len, const float *T, const float *p, const float *Y,
+                    const PostArgsHost &pa, cudaStream_t s) {
+    int rc = forward_chunk_bf16(c, n, a, len, T, p, Y, false, c->o_buf, c->chunk, s);
+    if (rc != GPUANN_OK) return rc;
+    CU_TRY(c, launch_post(c, n, a, len, pa.T, pa.Y, pa.h, c->o_buf, c->chunk, pa.dt, false, s), "update kernel");
+    return GPUANN_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -522,14 +537,60 @@ int gpuann_chem_step_host(gpuann_ctx *c, int64_t n, float *T, const float *p, fl
     float *dT = c->stage, *dp = dT + n, *dh = dp + n, *dY = dh + n;
     cudaStream_t s = c->own_stream;
     const size_t fb = (size_t)n * sizeof(float);
-    CU_TRY(c, cudaMemcpyAsync(dT, T, fb, cudaMemcpyHostToDevice, s), "H2D T");
-    CU_TRY(c, cudaMemcpyAsync(dp, p, fb, cudaMemcpyHostToDevice, s), "H2D p");
-    CU_TRY(c, cudaMemcpyAsync(dh, h, fb, cudaMemcpyHostToDevice, s), "H2D h");
-    CU_TRY(c, cudaMemcpyAsync(dY, Y, fb * Ns, cudaMemcpyHostToDevice, s), "H2D Y");
-    rc = gpuann_chem_step(c, n, dT, dp, dY, dh, dt, s);
-    if (rc != GPUANN_OK) return rc;
-    CU_TRY(c, cudaMemcpyAsync(T, dT, fb, cudaMemcpyDeviceToHost, s), "D2H T");
-    CU_TRY(c, cudaMemcpyAsync(Y, dY, fb * Ns, cudaMemcpyDeviceToHost, s), "D2H Y");
+    const bool pipelined = c->prm.precision == GPUANN_PRECISION_BF16 && !(c->prm.T_active > 0.0) && n >= 4 * 128 * (int64_t)c->sm_count;
+    if (!pipelined) {
+        CU_TRY(c, cudaMemcpyAsync(dT, T, fb, cudaMemcpyHostToDevice, s), "H2D T");
+        CU_TRY(c, cudaMemcpyAsync(dp, p, fb, cudaMemcpyHostToDevice, s), "H2D p");
+        CU_TRY(c, cudaMemcpyAsync(dh, h, fb, cudaMemcpyHostToDevice, s), "H2D h");
+        CU_TRY(c, cudaMemcpyAsync(dY, Y, fb * Ns, cudaMemcpyHostToDevice, s), "H2D Y");
+        rc = gpuann_chem_step(c, n, dT, dp, dY, dh, dt, s);
+        if (rc != GPUANN_OK) return rc;
+        CU_TRY(c, cudaMemcpyAsync(T, dT, fb, cudaMemcpyDeviceToHost, s), "D2H T");
+        CU_TRY(c, cudaMemcpyAsync(Y, dY, fb * Ns, cudaMemcpyDeviceToHost, s), "D2H Y");
+        CU_TRY(c, cudaStreamSynchronize(s), "cudaStreamSynchronize");
+        return GPUANN_OK;
+    }
+    // Pipelined: the field is cut into slices of whole tiles; slice i+1 is copied in and slice i-1 copied out (on two
+    // copy streams) while slice i is computed -- cells are independent, and the kernels take (first cell, count)
+    // of a field with row stride n, so a slice needs no repacking.  The step is then PCIe bound or compute bound,
+    // whichever is slower, instead of the sum.
+    constexpr int kMaxSlices = 16;
+    if (!c->copy_in) {
+        CU_TRY(c, cudaStreamCreateWithFlags(&c->copy_in, cudaStreamNonBlocking), "cudaStreamCreate");
+        CU_TRY(c, cudaStreamCreateWithFlags(&c->copy_out, cudaStreamNonBlocking), "cudaStreamCreate");
+        for (int i = 0; i < 2 * kMaxSlices; ++i) {
+            cudaEvent_t e;
+            CU_TRY(c, cudaEventCreateWithFlags(&e, cudaEventDisableTiming), "cudaEventCreate");
+            c->slice_events.push_back(e);
+        }
+    }
+    const int64_t unit = 128 * (int64_t)c->sm_count;
+    int64_t slice = ((n + 7) / 8 + unit - 1) / unit * unit;
+    if (slice > c->chunk) slice = c->chunk;
+    while ((n + slice - 1) / slice > kMaxSlices) slice += unit;
+    const size_t pitch = fb;
+    c->last_stream = s;
+    int i = 0;
+    for (int64_t a = 0; a < n; a += slice, ++i) {
+        const int64_t len = (n - a) < slice ? (n - a) : slice;
+        const size_t lb = (size_t)len * sizeof(float);
+        cudaEvent_t e_in = c->slice_events[2 * i], e_done = c->slice_events[2 * i + 1];
+        CU_TRY(c, cudaMemcpyAsync(dT + a, T + a, lb, cudaMemcpyHostToDevice, c->copy_in), "H2D T");
+        CU_TRY(c, cudaMemcpyAsync(dp + a, p + a, lb, cudaMemcpyHostToDevice, c->copy_in), "H2D p");
+        CU_TRY(c, cudaMemcpyAsync(dh + a, h + a, lb, cudaMemcpyHostToDevice, c->copy_in), "H2D h");
+        CU_TRY(c, cudaMemcpy2DAsync(dY + a, pitch, Y + a, pitch, lb, Ns, cudaMemcpyHostToDevice, c->copy_in), "H2D Y");
+        CU_TRY(c, cudaEventRecord(e_in, c->copy_in), "cudaEventRecord");
+        CU_TRY(c, cudaStreamWaitEvent(s, e_in, 0), "cudaStreamWaitEvent");
+        const PostArgsHost pa{dT, dY, dh, dt};
+        rc = step_slice_bf16(c, n, a, len, dT, dp, dY, pa, s);
+        if (rc != GPUANN_OK) return rc;
+        CU_TRY(c, cudaEventRecord(e_done, s), "cudaEventRecord");
+        CU_TRY(c, cudaStreamWaitEvent(c->copy_out, e_done, 0), "cudaStreamWaitEvent");
+        CU_TRY(c, cudaMemcpyAsync(T + a, dT + a, lb, cudaMemcpyDeviceToHost, c->copy_out), "D2H T");
+        CU_TRY(c, cudaMemcpy2DAsync(Y + a, pitch, dY + a, pitch, lb, Ns, cudaMemcpyDeviceToHost, c->copy_out), "D2H Y");
+    }
+    c->host_active += n;
+    CU_TRY(c, cudaStreamSynchronize(c->copy_out), "cudaStreamSynchronize");
     CU_TRY(c, cudaStreamSynchronize(s), "cudaStreamSynchronize");
     return GPUANN_OK;
 }
@@ -656,6 +717,10 @@ int gpuann_destroy(gpuann_ctx *c) {
         for (cudaEvent_t e : c->event_pool) cudaEventDestroy(e);
         c->event_pool.clear();
         if (c->own_stream) cudaStreamDestroy(c->own_stream);
+        if (c->copy_in) cudaStreamDestroy(c->copy_in);
+        if (c->copy_out) cudaStreamDestroy(c->copy_out);
+        for (cudaEvent_t e : c->slice_events) cudaEventDestroy(e);
+        c->slice_events.clear();
         cudaGetLastError();
     }
     delete c;

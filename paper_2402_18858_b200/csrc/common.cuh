@@ -129,6 +129,8 @@ struct Ctx {
     Counters *counters = nullptr;  // DEVICE
     int64_t host_active = 0;       // cells counted as active without a device-side compaction
     cudaStream_t own_stream = nullptr;  // used by gpuann_chem_step_host
+    cudaStream_t copy_in = nullptr, copy_out = nullptr;  // copy streams of the pipelined host variant
+    std::vector<cudaEvent_t> slice_events;
     cudaStream_t last_stream = nullptr;
     int64_t launches = 0;
 

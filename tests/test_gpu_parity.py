@@ -175,3 +175,25 @@ def test_abi_behaviour_on_device():
             assert e.value.status == B.GPUANN_ERR_INVALID_ARG
     finally:
         B.gpuann_destroy(ctx)
+
+
+@pytest.mark.parametrize("n", [128 * 9 + 5, 4 * 128 * 148 + 128 * 300 + 77])
+def test_host_variant_equals_device_variant(n):
+    """gpuann_chem_step_host (H2D + step + D2H inside; pipelined over slices for large n) returns bit for bit what
+    gpuann_chem_step returns on device-resident state."""
+    import torch
+    pr = G.prepare(I.get_config("c2"), n=n)
+    ctx = G.make_ctx(pr)
+    try:
+        dev = G.run_gpu(ctx, pr, want_raw=False)
+        st = pr.prob.state
+        Th = torch.from_numpy(st.T.copy()).pin_memory()
+        ph = torch.from_numpy(st.p.copy()).pin_memory()
+        Yh = torch.from_numpy(np.ascontiguousarray(st.Y).copy()).pin_memory()
+        hh = torch.from_numpy(pr.h.copy()).pin_memory()
+        B.gpuann_chem_step_host(ctx, n, Th.data_ptr(), ph.data_ptr(), Yh.data_ptr(), hh.data_ptr(), pr.prob.cfg.dt)
+        assert np.array_equal(Th.numpy().view(np.uint32), dev.T_new.view(np.uint32))
+        assert np.array_equal(Yh.numpy().view(np.uint32), dev.Y_new.view(np.uint32))
+        assert np.array_equal(ph.numpy(), st.p) and np.array_equal(hh.numpy(), pr.h)  # read-only inputs untouched
+    finally:
+        B.gpuann_destroy(ctx)

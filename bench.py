@@ -295,9 +295,15 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         flop_step = float(cfg.flop_per_cell) * n_act_per_step
     dom_ms_per_step = dom_ms / args.steps
     achieved = flop_step / (dom_ms_per_step * 1e-3) / 1e12
+    # DRAM bytes of the dominant kernel per launch from the committed ncu capture of exactly this configuration
+    # (profiles/r01_fused_l1l2.md, last section: dram__bytes_read.sum + dram__bytes_write.sum = 0.10 + 1.62 GB; the
+    # kernel writes h2 = 1,048,576 x 1,600 B once and reads the 96 MB of state once); null for any other configuration
+    traffic = None
+    if dom_name == "bf16_fused" and cfg.index == 2 and n == 1048576 and not args.chunk:
+        traffic = 1.725e9
     roofline = {
         "bound": "tensor", "kernel": dom_name, "achieved": achieved, "peak": peaks["bf16_tflops"], "unit": "TFLOP/s",
-        "frac": achieved / peaks["bf16_tflops"], "traffic": None, "peak_source": peak_src + ", burst",
+        "frac": achieved / peaks["bf16_tflops"], "traffic": traffic, "peak_source": peak_src + ", burst",
         "launches_per_step": dom_cnt / args.steps, "ms_per_step_in_kernel": dom_ms_per_step,
         "share_of_step": dom_ms_per_step / step_ms_sum if step_ms_sum > 0 else None,
         "flop_per_step_algorithmic": flop_step,

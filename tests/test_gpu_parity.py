@@ -197,3 +197,26 @@ def test_host_variant_equals_device_variant(n):
         assert np.array_equal(ph.numpy(), st.p) and np.array_equal(hh.numpy(), pr.h)  # read-only inputs untouched
     finally:
         B.gpuann_destroy(ctx)
+
+
+def test_experimental_split_variant_matches_oracle():
+    """GPUANN_FUSED=split (two CTAs per tile, layer-2 columns split over the cluster, h1 exchanged through distributed
+    shared memory; slower than the default, kept for round 2) must give the same parity.  The switch is read once per
+    process, so the case runs in a child process."""
+    import os
+    import subprocess
+    import sys
+    from pathlib import Path
+    root = Path(__file__).resolve().parents[1]
+    code = (
+        "import sys; sys.path.insert(0, %r); sys.path.insert(0, %r)\n"
+        "import gpu_common as G\n"
+        "from paper_2402_18858_b200 import inputs as I, binding as B\n"
+        "pr = G.prepare(I.get_config('c2'), n=128 * 11 + 29)\n"
+        "ctx = G.make_ctx(pr, chunk_cells=1024)\n"
+        "g = G.run_gpu(ctx, pr); ref = G.run_oracle(pr)\n"
+        "G.check_raw_bf16(g.o_raw, ref.o_raw); G.check_T_bf16(g, ref); G.check_sumY(g.Y_new)\n"
+        "B.gpuann_destroy(ctx); print('SPLIT-OK')\n" % (str(root), str(root / "tests")))
+    env = dict(os.environ, GPUANN_FUSED="split")
+    r = subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, timeout=300)
+    assert r.returncode == 0 and "SPLIT-OK" in r.stdout, r.stdout + r.stderr

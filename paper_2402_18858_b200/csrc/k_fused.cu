@@ -38,6 +38,7 @@ constexpr int kL1Slots = 3;
 constexpr int kAccCols = 416;    // TMEM columns of the layer-2 accumulator (max pass width)
 constexpr int kL1Col = kAccCols; // L1 slots live in columns 416..511
 constexpr int kFusedThreads = 512;
+constexpr int kSplitThreads = 544;  // k_fused_split: + one forwarder warp
 
 constexpr uint32_t kW2StageBytes = kAccCols * 128;  // 53,248
 constexpr uint32_t kW1StageBytes = kFK * 128;       // 8,192
@@ -57,7 +58,7 @@ enum {
     bW2Full = 0, bW2Empty = bW2Full + kW2Stages, bW1Full = bW2Empty + kW2Stages, bW1Empty = bW1Full + kW1Stages,
     bAFull = bW1Empty + kW1Stages, bAEmpty = bAFull + kAStages, bL1Full = bAEmpty + kAStages,
     bL1Empty = bL1Full + kL1Slots, bZFull = bL1Empty + kL1Slots, bZEmpty = bZFull + 2, bAccFull = bZEmpty + 2,
-    bAccEmpty = bAccFull + 1, bCount = bAccEmpty + 1
+    bAccEmpty = bAccFull + 1, bAFullR = bAccEmpty + 1 /* k_fused_split: chunks forwarded by the peer */, bCount = bAFullR + kAStages
 };
 
 struct FusedArgs {
@@ -439,14 +440,15 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
 // k_fused_split -- the same job for nets whose layer 2 needs two passes (H2p in (kAccCols, 2 kAccCols]): the two CTAs of
 // a cluster work on the SAME 128-cell tile and split the layer-2 columns: CTA r accumulates columns [r pass_w, ...) over
 // the full K = H1 -- no passes, so h1 is computed once per tile instead of once per pass.  The h1 chunks are split too:
-// chunk g (global chunk counter) is produced by CTA g & 1 (layer-1 MMA, tcgen05.ld, GELU, BF16) and written into the A
-// ring of BOTH CTAs (local st.shared + st.shared::cluster to the peer).  Per CTA and tile: 25 chunks of layer-2 MMAs
+// chunk g (global chunk counter) is produced by CTA g & 1 (layer-1 MMA, tcgen05.ld, GELU, BF16) into its own A ring and
+// forwarded to the peer's A ring by one bulk copy through distributed shared memory (warp 16).  Per CTA and tile: 25 chunks of layer-2 MMAs
 // (800 clk each), 12-13 chunks of layer-1 MMAs and h1 GELU, ONE accumulator drain -- against 50 + 50 + 2 before.
-//   AFull[s]   in each CTA: 8 arrivals from the producer warps of the CTA that owns the chunk (local or remote arrive)
+//   AFull[s]   own chunks: 8 arrivals from the local producer warps;  AFullR[s]  the peer's chunks: expect_tx + 16 KB
+//              of the peer forwarder's cp.async.bulk.shared::cluster
 //   AEmpty[s]  in each CTA: 2 tcgen05.commit arrivals (own layer-2 issuer + the peer's, multicast): a stage is rewritten
 //              only when BOTH CTAs' MMAs have read it
 // Everything else (weight rings, layer-1 slots, z, accumulator hand-over) is local to a CTA.
-__global__ void __launch_bounds__(kFusedThreads, 1)
+__global__ void __launch_bounds__(kSplitThreads, 1)
 k_fused_split(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__ CUtensorMap tmapW2a,
               const __grid_constant__ CUtensorMap tmapW2b, const FusedArgs fa) {
     extern __shared__ unsigned char smem_raw[];
@@ -476,7 +478,11 @@ k_fused_split(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant_
     if (threadIdx.x == 0) {
         for (int i = 0; i < kW2Stages; ++i) { ptx::mbar_init(&bars[bW2Full + i], 1); ptx::mbar_init(&bars[bW2Empty + i], 1); }
         for (int i = 0; i < kW1Stages; ++i) { ptx::mbar_init(&bars[bW1Full + i], 1); ptx::mbar_init(&bars[bW1Empty + i], 1); }
-        for (int i = 0; i < kAStages; ++i) { ptx::mbar_init(&bars[bAFull + i], 8); ptx::mbar_init(&bars[bAEmpty + i], 2); }
+        for (int i = 0; i < kAStages; ++i) {
+            ptx::mbar_init(&bars[bAFull + i], 8);    // own chunks: the 8 producer warps
+            ptx::mbar_init(&bars[bAFullR + i], 1);   // the peer's chunks: its forwarder's expect_tx + 16 KB of bulk copy
+            ptx::mbar_init(&bars[bAEmpty + i], 2);
+        }
         for (int i = 0; i < kL1Slots; ++i) { ptx::mbar_init(&bars[bL1Full + i], 1); ptx::mbar_init(&bars[bL1Empty + i], 4); }
         for (int i = 0; i < 2; ++i) { ptx::mbar_init(&bars[bZFull + i], 1); ptx::mbar_init(&bars[bZEmpty + i], 1); }
         ptx::mbar_init(&bars[bAccFull], 1);
@@ -538,13 +544,22 @@ k_fused_split(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant_
         const uint32_t idesc_n1 = ptx::umma_idesc_bf16_f32(kFM, (uint32_t)(fa.n1 > 0 ? fa.n1 : 16));
         const uint64_t b1_off = (uint64_t)((uint32_t)fa.n0 * 128u >> 4);
         Ring a, w2;
-        uint32_t acc_ph = 0;
+        uint32_t acc_ph = 0, own_ph = 0, rem_ph = 0;  // per-stage phase bits of AFull / AFullR
         for (int it = 0; it < my_tiles; ++it) {
             ptx::mbar_wait(&bars[bAccEmpty], acc_ph ^ 1u);
             ptx::tc_fence_after_sync();
             for (int c = 0; c < n_chunks; ++c) {
                 ptx::mbar_wait(&bars[bW2Full + w2.st], w2.ph);
-                ptx::mbar_wait_cluster(&bars[bAFull + a.st], a.ph);  // half of the chunks were written by the peer
+                {   // own chunks complete AFull (local producers), the peer's chunks AFullR (its forwarder's bulk copy)
+                    const uint32_t bit = 1u << a.st;
+                    if ((uint32_t)((it * n_chunks + c) & 1) == crank) {
+                        ptx::mbar_wait(&bars[bAFull + a.st], (own_ph & bit) ? 1u : 0u);
+                        own_ph ^= bit;
+                    } else {
+                        ptx::mbar_wait_cluster(&bars[bAFullR + a.st], (rem_ph & bit) ? 1u : 0u);
+                        rem_ph ^= bit;
+                    }
+                }
                 ptx::tc_fence_after_sync();
                 const uint64_t da = desc0 + (uint64_t)((kOffA + a.st * kAStageBytes) >> 4);
                 const uint64_t db = desc0 + (uint64_t)((kOffW2 + w2.st * kW2StageBytes) >> 4);
@@ -684,8 +699,6 @@ k_fused_split(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant_
         const uint32_t row_off = (uint32_t)r * 128u;
         uint32_t slot = (uint32_t)set, slot_ph = 0;  // own sub-chunk j = 2 (own chunk ordinal) + set: slot j % 3, phase (j / 3) & 1
         uint32_t ast = crank % 3, a_ph = 0;          // A stage / phase of global chunk g = crank, crank + 2, ...
-        const uint32_t a_full_peer = ptx::mapa_u32(ptx::smem_u32(&bars[bAFull]), peer);
-        const uint32_t a_ring_peer = ptx::mapa_u32(sbase + kOffA, peer);
 #pragma unroll 1
         for (int g = (int)crank; g < total; g += 2) {
             ptx::mbar_wait(&bars[bL1Full + slot], slot_ph);
@@ -705,14 +718,10 @@ k_fused_split(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant_
             for (int i = 0; i < 4; ++i) {
                 const uint32_t u = ((((uint32_t)(4 * set + i)) ^ swz) << 4);
                 ptx::st_shared_v4(sbase + kOffA + off + u, o[4 * i], o[4 * i + 1], o[4 * i + 2], o[4 * i + 3]);
-                ptx::st_cluster_v4(a_ring_peer + off + u, o[4 * i], o[4 * i + 1], o[4 * i + 2], o[4 * i + 3]);
             }
-            ptx::fence_proxy_async_all();
+            ptx::fence_proxy_async_smem();  // the MMA and the forwarder's bulk copy read through the async proxy
             __syncwarp();
-            if (lane == 0) {
-                ptx::mbar_arrive(&bars[bAFull + ast]);
-                ptx::mbar_arrive_cluster(a_full_peer + ast * 8u);
-            }
+            if (lane == 0) ptx::mbar_arrive(&bars[bAFull + ast]);
             ast += 2;  // g += 2
             if (ast >= 3) {
                 ast -= 3;
@@ -722,6 +731,26 @@ k_fused_split(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant_
             if (slot >= kL1Slots) {
                 slot -= kL1Slots;
                 slot_ph ^= 1u;
+            }
+        }
+    } else if (warp == 16) {
+        // ================================================================ forwarder: own finished A stages -> the peer's A ring
+        // one bulk copy (async proxy, 16 KB) per own chunk, completing on the peer's AFullR barrier; the producers
+        // then pay no remote stores and no cluster-scope fence (those cost ~3,000 clk per chunk, profiles/)
+        if (lane == 0) {
+            uint32_t own_ph = 0;
+            uint32_t ast = crank % 3;
+            const uint32_t ring_peer = ptx::mapa_u32(sbase + kOffA, peer);
+            const uint32_t full_r_peer = ptx::mapa_u32(ptx::smem_u32(&bars[bAFullR]), peer);
+            for (int g = (int)crank; g < total; g += 2) {
+                const uint32_t bit = 1u << ast;
+                ptx::mbar_wait(&bars[bAFull + ast], (own_ph & bit) ? 1u : 0u);
+                own_ph ^= bit;
+                ptx::mbar_arrive_expect_tx_cluster(full_r_peer + ast * 8u, kAStageBytes);
+                ptx::bulk_copy_to_cluster(ring_peer + ast * kAStageBytes, sbase + kOffA + ast * kAStageBytes, kAStageBytes,
+                                          full_r_peer + ast * 8u);
+                ast += 2;
+                if (ast >= 3) ast -= 3;
             }
         }
     } else {
@@ -858,13 +887,14 @@ cudaError_t launch_fused_l1l2(Ctx *c, int64_t n, int64_t c0, int64_t cn, const f
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    // EXPERIMENTAL (GPUANN_FUSED=split): correct, but 3.98 ms against 2.70 ms per 1 M cells -- every h1 chunk pays ~3,000 clk
-    // of fence.proxy.async + release-arrive latency after its st.shared::cluster stores (profiles/r01_fused_l1l2.md)
+    // EXPERIMENTAL (GPUANN_FUSED=split): correct, but 2.92 ms against 2.70 ms per 1 M cells -- the 16 KB per chunk that the
+    // pair exchanges through distributed shared memory is the bound (profiles/r01_fused_l1l2.md)
     static const bool split = [] { const char *e = std::getenv("GPUANN_FUSED"); return e && std::strcmp(e, "split") == 0; }();
     if (fn.n_pass == 2 && split) {
         // two CTAs per tile: as many clusters as there are tiles, at most one per pair of SMs
         int pairs = (int)(tiles < c->sm_count / 2 ? tiles : c->sm_count / 2);
         cfg.gridDim = dim3((unsigned)(2 * pairs));
+        cfg.blockDim = dim3(kSplitThreads);
         return cudaLaunchKernelEx(&cfg, k_fused_split, fn.tmapW1, fn.tmapW2a, fn.tmapW2b, fa);
     }
     return cudaLaunchKernelEx(&cfg, k_fused_l1l2, fn.tmapW1, fn.tmapW2a, fn.tmapW2b, fa);

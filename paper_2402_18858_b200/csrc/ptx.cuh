@@ -12,12 +12,6 @@ __device__ __forceinline__ uint32_t smem_u32(const void *p) {
     return static_cast<uint32_t>(__cvta_generic_to_shared(p));
 }
 
-__device__ __forceinline__ uint32_t lane_id() {
-    uint32_t l;
-    asm volatile("mov.u32 %0, %%laneid;" : "=r"(l));
-    return l;
-}
-
 __device__ __forceinline__ bool elect_one() {
     uint32_t pred;
     asm volatile(
@@ -99,28 +93,6 @@ __device__ __forceinline__ void tma_load_2d(const void *tmap, uint64_t *bar, voi
         : "memory");
 }
 
-// the same with an L2 cache-policy operand (createpolicy result)
-__device__ __forceinline__ void tma_load_2d_hint(const void *tmap, uint64_t *bar, void *smem_dst, int32_t c0,
-                                                 int32_t c1, uint64_t policy) {
-    asm volatile(
-        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint"
-        " [%0], [%1, {%3, %4}], [%2], %5;" ::"r"(smem_u32(smem_dst)),
-        "l"(reinterpret_cast<uint64_t>(tmap)), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "l"(policy)
-        : "memory");
-}
-
-__device__ __forceinline__ uint64_t policy_evict_last() {
-    uint64_t p;
-    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
-    return p;
-}
-
-__device__ __forceinline__ uint64_t policy_evict_first() {
-    uint64_t p;
-    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
-    return p;
-}
-
 // ---------------------------------------------------------------- thread-block clusters (pairs of CTAs)
 __device__ __forceinline__ uint32_t cluster_ctarank() {
     uint32_t r;
@@ -137,13 +109,6 @@ __device__ __forceinline__ uint32_t mapa_u32(uint32_t local_smem_addr, uint32_t 
     uint32_t r;
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local_smem_addr), "r"(cta));
     return r;
-}
-__device__ __forceinline__ void st_cluster_v4(uint32_t cluster_addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
-    asm volatile("st.shared::cluster.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(cluster_addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
-}
-// arrive (release at cluster scope) on an mbarrier given by its shared::cluster address (own or peer CTA)
-__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
-    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
 }
 // arrive + expect_tx on an mbarrier given by its shared::cluster address (own or peer CTA)
 __device__ __forceinline__ void mbar_arrive_expect_tx_cluster(uint32_t cluster_addr, uint32_t bytes) {
@@ -173,8 +138,6 @@ __device__ __forceinline__ void mbar_wait_cluster(uint64_t *bar, uint32_t parity
             : "memory");
     } while (!ok);
 }
-// generic-proxy writes (any state space, incl. the peer's shared memory) -> visible to the async proxy
-__device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.proxy.async.shared::cluster;" ::: "memory"); }
 
 // TMA tile load delivered to the same shared-memory offset of every CTA in cta_mask; each destination CTA's
 // mbarrier at the same offset as `bar` receives the complete_tx of the bytes that landed in ITS shared memory
@@ -255,32 +218,6 @@ __device__ __forceinline__ void umma_bf16_ss(uint32_t tmem_d, uint64_t desc_a, u
 __device__ __forceinline__ void umma_commit(uint64_t *bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar))
                  : "memory");
-}
-
-// The same, executed by a whole (converged) warp: only the lane with elected != 0 issues.  Keeping the MMA
-// warp's control flow warp-uniform lets ptxas build descriptors in the uniform datapath (a few U-ops per MMA)
-// instead of ~20 vector ops + R2UR per MMA inside an `if (lane == 0)` branch (profiles/r01: issue-bound).
-__device__ __forceinline__ void umma_bf16_ss_pred(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b, uint32_t idesc,
-                                                  uint32_t accumulate, uint32_t elected) {
-    asm volatile(
-        "{\n\t"
-        ".reg .pred p, q;\n\t"
-        "setp.ne.b32 p, %4, 0;\n\t"
-        "setp.ne.b32 q, %5, 0;\n\t"
-        "@q tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t"
-        "}\n" ::"r"(tmem_d),
-        "l"(desc_a), "l"(desc_b), "r"(idesc), "r"(accumulate), "r"(elected)
-        : "memory");
-}
-__device__ __forceinline__ void umma_commit_pred(uint64_t *bar, uint32_t elected) {
-    asm volatile(
-        "{\n\t"
-        ".reg .pred q;\n\t"
-        "setp.ne.b32 q, %1, 0;\n\t"
-        "@q tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n\t"
-        "}\n" ::"r"(smem_u32(bar)),
-        "r"(elected)
-        : "memory");
 }
 
 // ---------------------------------------------------------------- tcgen05: TMEM -> registers

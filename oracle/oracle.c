@@ -25,7 +25,9 @@
  * Pins (tests/test_oracle_*.py): Eq. 7 end points f(0) = -1/lambda, f(1) = 0
  * (PAPER.md:103), lambda -> 0 limit, round trip; GELU textbook constants and an
  * independent numpy/scipy evaluation; hand-expanded tiny nets; closed-form and
- * brentq Newton roots; sum(Y) = 1; zero-net fixed point; permutation invariance.
+ * brentq Newton roots; sum(Y) = 1; zero-net fixed point; permutation invariance;
+ * o_raw from an independently built z (feature order, division by sigma); mu_out != 0;
+ * T == 600.0f boundary; vanishing-sum fallback; cp <= 0 stop; clamped Newton start.
  * Parity unpinned: R3 (what the de-normalised output means) and R5 (erf vs tanh
  * GELU) are choices the paper does not settle; they are fixed by DESIGN.md.
  */

@@ -373,6 +373,137 @@ def test_step_active_threshold_skips_cold_cells_bit_identically():
     assert np.array_equal(ra.T_new, r.T_new[act]) and np.array_equal(ra.Y_new, r.Y_new[:, act])
 
 
+# ------------------------------------------------------------------ pins added in round 2 ("What's weak" #1)
+# Each docstring names the mutation of oracle.c that it catches (all of them passed the round-1 pins).
+def _numpy_net(net, z):
+    """numpy / scipy MLP on columns of z ([D][m]); exact-erf GELU on hidden layers."""
+    a = z
+    L = len(net.weights)
+    for l, (W, b) in enumerate(zip(net.weights, net.biases)):
+        a = W.astype(np.float64) @ a + b.astype(np.float64)[:, None]
+        if l < L - 1:
+            a = 0.5 * a * (1.0 + special.erf(a / math.sqrt(2.0)))
+    return a
+
+
+def test_step_raw_output_from_independently_built_z():
+    """PAPER.md:98 (input = {T, p, F(Y)} in this order), R4 (z = (x - mu)/sigma).  z is built here with numpy / scipy
+    alone and pushed through a numpy / scipy MLP; chem_step's o_raw must agree to 1e-12.
+    Catches: `* in_std` for `/ in_std` at O2; T and p swapped at O2; y_k fed in the wrong slot."""
+    pr, h, m = _small_problem("c0", n=16, seed=41)
+    st = pr.state
+    # statistics that are NOT symmetric between T, p and the species, and sigma far from 1
+    rng = np.random.default_rng(5)
+    m.in_mean = (np.asarray(m.in_mean) + rng.normal(size=11).astype(np.float32) * np.asarray(m.in_std)).astype(np.float32)
+    m.in_std = (np.asarray(m.in_std) * rng.uniform(0.5, 3.0, 11)).astype(np.float32)
+    r = oracle.Oracle(m).chem_step(st.T, st.p, st.Y, h, 1e-6)
+    x = np.vstack([st.T.astype(np.float64), st.p.astype(np.float64),
+                   special.boxcox(np.maximum(st.Y.astype(np.float64), 0.0), 0.1)])
+    z = (x - m.in_mean.astype(np.float64)[:, None]) / m.in_std.astype(np.float64)[:, None]
+    want = _numpy_net(pr.net, z)
+    assert np.allclose(r.o_raw, want, rtol=1e-12, atol=1e-12)
+    # the test has teeth: swapping the first two features or multiplying by sigma changes the output
+    zs = z.copy()
+    zs[[0, 1]] = zs[[1, 0]]
+    assert np.abs(_numpy_net(pr.net, zs) - want).max() > 1e-3
+
+
+def test_step_nonzero_output_mean_enters_with_plus_sign():
+    """R3: dy = dt (o sigma_out + mu_out).  mu_out = +-5e3 1/s per species; Y_new recomputed through scipy's
+    inv_boxcox from the oracle's own o_raw.  Catches: `- out_mean` at O4, mu_out dropped, mu_out not scaled by dt."""
+    pr, h, m = _small_problem("c0", n=48, seed=43)
+    st = pr.state
+    mu = np.array([5e3 if k % 2 == 0 else -5e3 for k in range(9)], dtype=np.float32) * np.linspace(0.5, 1.5, 9).astype(np.float32)
+    m.out_mean = mu
+    dt = 1e-6
+    r = oracle.Oracle(m).chem_step(st.T, st.p, st.Y, h, dt)
+    y = special.boxcox(np.maximum(st.Y.astype(np.float64), 0.0), 0.1)
+    dy = dt * (r.o_raw * m.out_std.astype(np.float64)[:, None] + mu.astype(np.float64)[:, None])
+    Ystar = special.inv_boxcox(y + dy, 0.1)
+    want = Ystar / Ystar.sum(axis=0)
+    assert np.allclose(r.Y_new, want, rtol=1e-11, atol=1e-300)
+    wrong = special.inv_boxcox(y + dt * (r.o_raw * m.out_std.astype(np.float64)[:, None] - mu.astype(np.float64)[:, None]), 0.1)
+    assert np.abs(wrong / wrong.sum(axis=0) - want).max() > 1e-6     # the sign matters at this size of mu_out
+
+
+def test_step_threshold_boundary_600_is_active():
+    """R12: FP32 `T < 600.0f` means skipped, so T == 600.0f is ACTIVE and nextafter(600, 0) is skipped.
+    Catches: `<=` for `<` at O0."""
+    pr, h, m = _small_problem("c4", n=64, seed=47)
+    st = pr.state
+    T = st.T.copy()
+    T[0] = np.float32(600.0)
+    T[1] = np.nextafter(np.float32(600.0), np.float32(0.0))
+    T[2] = np.nextafter(np.float32(600.0), np.float32(1e9))
+    th = pr.thermo
+    h2 = oracle.enthalpy_field(T, st.Y, th.nasa_lo, th.nasa_hi, th.T_mid, th.W).astype(np.float32)
+    r = oracle.Oracle(m).chem_step(T, st.p, st.Y, h2, 1e-6)
+    assert r.flags[0] != 4 and r.flags[2] != 4 and r.flags[1] == 4
+    assert r.iters[0] >= 1 and np.abs(r.Y_new[:, 0].sum() - 1.0) < 1e-14
+    assert np.array_equal(r.Y_new[:, 1], st.Y[:, 1].astype(np.float64)) and r.T_new[1] == float(T[1])
+    assert not np.array_equal(r.Y_new[:, 0], st.Y[:, 0].astype(np.float64))     # cell 0 was really stepped
+
+
+def test_step_vanishing_sum_falls_back_to_clamped_input_over_its_sum():
+    """R8: every 1 + lambda (y + dy) <= 0 (mu_out = -1e8 1/s => dy = -100)  =>  Y_new = Yc / sum(Yc), flag bit 1.
+    The inputs do NOT sum to one (and hold a negative entry), so the division by sum(Yc) is visible.
+    Catches: the fallback without `/ Sc`, Y instead of Yc in the fallback, the flag not set."""
+    pr, h, m = _small_problem("c0", n=12, seed=53)
+    st = pr.state
+    Y = (st.Y * np.float32(0.8)).astype(np.float32)
+    Y[3, :] = -1e-4
+    m.out_mean = np.full(9, -1e8, dtype=np.float32)
+    r = oracle.Oracle(m).chem_step(st.T, st.p, Y, h, 1e-6)
+    Yc = np.maximum(Y.astype(np.float64), 0.0)
+    assert np.allclose(r.Y_new, Yc / Yc.sum(axis=0), rtol=1e-15, atol=0)
+    assert np.all(r.Y_new[3] == 0.0) and np.all((r.flags & 2) == 2)
+    assert np.all(np.abs(Yc.sum(axis=0) - 1.0) > 0.1)
+
+
+def test_newton_stops_at_once_when_cp_is_not_positive():
+    """R10: c = sum Y_k cp_k <= 0 at the (clamped) start  =>  no update, 0 iterations, not converged, T = start.
+    Catches: the `if (!(c > 0)) break` removed (the iteration would then walk away on a negative slope)."""
+    th = _thermo(4, 13)
+    lo = th.nasa_lo.copy()
+    lo[:, 0] = -np.abs(lo[:, 0])          # a1 < 0 and a2..a5 small: cp < 0 on the whole range
+    lo[:, 1:5] = 0.0
+    Y = np.array([0.25, 0.25, 0.25, 0.25])
+    assert oracle.mixture_cp(Y, 900.0, lo, None, None, th.W) < 0.0
+    h = oracle.mixture_h(Y, 1200.0, lo, None, None, th.W)
+    T, it, conv = oracle.newton_T(Y, h, 900.0, lo, None, None, th.W)
+    assert T == 900.0 and it == 0 and not conv
+    # and through the whole step: flag bit 0 set, T_new = the incoming T
+    pr, hh, m = _small_problem("c0", n=8, seed=59)
+    lo9 = pr.thermo.nasa_lo.copy()
+    lo9[:, 0] = -np.abs(lo9[:, 0])
+    lo9[:, 1:5] = 0.0
+    m.nasa_lo = lo9
+    r = oracle.Oracle(m).chem_step(pr.state.T, pr.state.p, pr.state.Y, hh, 1e-6)
+    assert np.all(r.iters == 0) and np.all((r.flags & 1) == 1)
+    assert np.array_equal(r.T_new, pr.state.T.astype(np.float64))
+
+
+def test_newton_first_iterate_is_evaluated_at_the_clamped_start():
+    """R10: T_0 = clamp(T_start, T_min, T_max).  One update from T_start = 100 K / 5000 K must equal one update
+    written out by hand from 200 K / 3500 K on a QUADRATIC h(T) (a linear one lands on the root from anywhere).
+    Catches: the start clamp removed."""
+    th = _thermo(5, 17)
+    lo = th.nasa_lo.copy()
+    lo[:, 2:5] = 0.0
+    Y = np.array([0.1, 0.3, 0.2, 0.15, 0.25])
+    s = RU / th.W
+    A, Bq, Cc = float(np.sum(Y * s * lo[:, 0])), float(np.sum(Y * s * lo[:, 1])), float(np.sum(Y * s * lo[:, 5]))
+    hq = lambda T: A * T + Bq * T * T / 2 + Cc
+    cq = lambda T: A + Bq * T
+    h = hq(1500.0)
+    for T_start, T0 in ((100.0, 200.0), (5000.0, 3500.0)):
+        want = T0 - (hq(T0) - h) / cq(T0)
+        T, it, conv = oracle.newton_T(Y, h, T_start, lo, None, None, th.W, max_iter=1)
+        assert it == 1 and not conv and abs(T - want) < 1e-9
+        unclamped = T_start - (hq(T_start) - h) / cq(T_start)
+        assert abs(unclamped - want) > 1.0               # so a missing clamp cannot pass
+
+
 def test_paper_speedup_arithmetic():
     """context numbers in BASELINE.md are self-consistent (ratio = 32/(1 - reduction))."""
     for red, ratio in read_golden("speedup_arithmetic.txt"):

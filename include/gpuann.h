@@ -131,7 +131,8 @@ int gpuann_chem_step(gpuann_ctx *ctx, int64_t n_cells, float *T, const float *p,
 /* The same step for a caller whose state lives in HOST memory: copies T, p, Y, h to the device
  * (library-owned staging buffers, grown lazily), runs gpuann_chem_step, copies T and Y back and
  * synchronises.  Pinned host memory makes the copies asynchronous.  On the BF16 path without an active-cell
- * threshold and for n_cells >= 4 tiles per SM the field is cut into <= 16 slices of whole tiles and slice i+1 is
+ * threshold and for n_cells >= 4 tiles per SM the field is cut into slices of whole tiles (about eight, never
+ * larger than the scratch chunk) and slice i+1 is
  * copied in / slice i-1 copied out on two copy streams while slice i is computed, so the call is bound by the
  * slower of PCIe and compute instead of their sum; the result is bit for bit that of gpuann_chem_step.
  * Arguments as gpuann_chem_step but HOST pointers.  This is the end-to-end entry bench.py times ("e2e"). */

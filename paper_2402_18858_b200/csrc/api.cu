@@ -255,10 +255,8 @@ int gpuann_load_net(gpuann_ctx *c, int n_species, int n_layers, const int *sizes
 
     // ---- BF16 tensor path: pad, round (RNE), upload, encode the tensor maps
     // variant: "bf16-fused" (S1 + S2 + layers 1-2 in one kernel, k_fused.cu) when the shapes allow it, else
-    // "bf16-layerwise".  GPUANN_VARIANT=layerwise forces the latter (A/B measurements).
-    const char *force = std::getenv("GPUANN_VARIANT");
-    const bool want_fused = !(force && std::strcmp(force, "layerwise") == 0);
-    const bool fused = want_fused && n_layers >= 3 && fused_supported(sizes[0], sizes[1], pad16(sizes[2]));
+    // "bf16-layerwise"
+    const bool fused = n_layers >= 3 && fused_supported(sizes[0], sizes[1], pad16(sizes[2]));
     int64_t chunk = c->prm.chunk_cells > 0 ? c->prm.chunk_cells : (int64_t)c->sm_count * 128 * (fused ? 56 : 1);
     chunk = (chunk + 127) / 128 * 128;
     c->chunk = chunk;
@@ -553,42 +551,67 @@ int gpuann_chem_step_host(gpuann_ctx *c, int64_t n, float *T, const float *p, fl
     // Pipelined: the field is cut into slices of whole tiles; slice i+1 is copied in and slice i-1 copied out (on two
     // copy streams) while slice i is computed -- cells are independent, and the kernels take (first cell, count)
     // of a field with row stride n, so a slice needs no repacking.  The step is then PCIe bound or compute bound,
-    // whichever is slower, instead of the sum.
-    constexpr int kMaxSlices = 16;
-    if (!c->copy_in) {
-        CU_TRY(c, cudaStreamCreateWithFlags(&c->copy_in, cudaStreamNonBlocking), "cudaStreamCreate");
-        CU_TRY(c, cudaStreamCreateWithFlags(&c->copy_out, cudaStreamNonBlocking), "cudaStreamCreate");
-        for (int i = 0; i < 2 * kMaxSlices; ++i) {
-            cudaEvent_t e;
-            CU_TRY(c, cudaEventCreateWithFlags(&e, cudaEventDisableTiming), "cudaEventCreate");
-            c->slice_events.push_back(e);
-        }
-    }
+    // whichever is slower, instead of the sum.  INVARIANT: a slice never exceeds the scratch chunk.
     const int64_t unit = 128 * (int64_t)c->sm_count;
     int64_t slice = ((n + 7) / 8 + unit - 1) / unit * unit;
     if (slice > c->chunk) slice = c->chunk;
-    while ((n + slice - 1) / slice > kMaxSlices) slice += unit;
+    const int64_t n_slices = (n + slice - 1) / slice;
+    if (!c->copy_in || !c->copy_out) {  // both streams or neither
+        cudaStream_t a = nullptr, b = nullptr;
+        cudaError_t e = cudaStreamCreateWithFlags(&a, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&b, cudaStreamNonBlocking);
+        if (e != cudaSuccess) {
+            if (a) cudaStreamDestroy(a);
+            if (b) cudaStreamDestroy(b);
+            return fail_cuda(c, e, "cudaStreamCreate");
+        }
+        c->copy_in = a;
+        c->copy_out = b;
+    }
+    while ((int64_t)c->slice_events.size() < 2 * n_slices) {
+        cudaEvent_t e;
+        CU_TRY(c, cudaEventCreateWithFlags(&e, cudaEventDisableTiming), "cudaEventCreate");
+        c->slice_events.push_back(e);
+    }
     const size_t pitch = fb;
     c->last_stream = s;
-    int i = 0;
+    // any failure inside the loop: wait for the copies already in flight into the caller's buffers, then report
+    auto drain = [&]() {
+        cudaStreamSynchronize(c->copy_in);
+        cudaStreamSynchronize(s);
+        cudaStreamSynchronize(c->copy_out);
+    };
+#define CU_TRY_DRAIN(call, what)                  \
+    do {                                          \
+        cudaError_t e__ = (call);                 \
+        if (e__ != cudaSuccess) {                 \
+            drain();                              \
+            return fail_cuda(c, e__, what);       \
+        }                                         \
+    } while (0)
+    int64_t i = 0;
     for (int64_t a = 0; a < n; a += slice, ++i) {
         const int64_t len = (n - a) < slice ? (n - a) : slice;
         const size_t lb = (size_t)len * sizeof(float);
         cudaEvent_t e_in = c->slice_events[2 * i], e_done = c->slice_events[2 * i + 1];
-        CU_TRY(c, cudaMemcpyAsync(dT + a, T + a, lb, cudaMemcpyHostToDevice, c->copy_in), "H2D T");
-        CU_TRY(c, cudaMemcpyAsync(dp + a, p + a, lb, cudaMemcpyHostToDevice, c->copy_in), "H2D p");
-        CU_TRY(c, cudaMemcpyAsync(dh + a, h + a, lb, cudaMemcpyHostToDevice, c->copy_in), "H2D h");
-        CU_TRY(c, cudaMemcpy2DAsync(dY + a, pitch, Y + a, pitch, lb, Ns, cudaMemcpyHostToDevice, c->copy_in), "H2D Y");
-        CU_TRY(c, cudaEventRecord(e_in, c->copy_in), "cudaEventRecord");
-        CU_TRY(c, cudaStreamWaitEvent(s, e_in, 0), "cudaStreamWaitEvent");
+        CU_TRY_DRAIN(cudaMemcpyAsync(dT + a, T + a, lb, cudaMemcpyHostToDevice, c->copy_in), "H2D T");
+        CU_TRY_DRAIN(cudaMemcpyAsync(dp + a, p + a, lb, cudaMemcpyHostToDevice, c->copy_in), "H2D p");
+        CU_TRY_DRAIN(cudaMemcpyAsync(dh + a, h + a, lb, cudaMemcpyHostToDevice, c->copy_in), "H2D h");
+        CU_TRY_DRAIN(cudaMemcpy2DAsync(dY + a, pitch, Y + a, pitch, lb, Ns, cudaMemcpyHostToDevice, c->copy_in), "H2D Y");
+        CU_TRY_DRAIN(cudaEventRecord(e_in, c->copy_in), "cudaEventRecord");
+        CU_TRY_DRAIN(cudaStreamWaitEvent(s, e_in, 0), "cudaStreamWaitEvent");
         const PostArgsHost pa{dT, dY, dh, dt};
         rc = step_slice_bf16(c, n, a, len, dT, dp, dY, pa, s);
-        if (rc != GPUANN_OK) return rc;
-        CU_TRY(c, cudaEventRecord(e_done, s), "cudaEventRecord");
-        CU_TRY(c, cudaStreamWaitEvent(c->copy_out, e_done, 0), "cudaStreamWaitEvent");
-        CU_TRY(c, cudaMemcpyAsync(T + a, dT + a, lb, cudaMemcpyDeviceToHost, c->copy_out), "D2H T");
-        CU_TRY(c, cudaMemcpy2DAsync(Y + a, pitch, dY + a, pitch, lb, Ns, cudaMemcpyDeviceToHost, c->copy_out), "D2H Y");
+        if (rc != GPUANN_OK) {
+            drain();
+            return rc;
+        }
+        CU_TRY_DRAIN(cudaEventRecord(e_done, s), "cudaEventRecord");
+        CU_TRY_DRAIN(cudaStreamWaitEvent(c->copy_out, e_done, 0), "cudaStreamWaitEvent");
+        CU_TRY_DRAIN(cudaMemcpyAsync(T + a, dT + a, lb, cudaMemcpyDeviceToHost, c->copy_out), "D2H T");
+        CU_TRY_DRAIN(cudaMemcpy2DAsync(Y + a, pitch, dY + a, pitch, lb, Ns, cudaMemcpyDeviceToHost, c->copy_out), "D2H Y");
     }
+#undef CU_TRY_DRAIN
     c->host_active += n;
     CU_TRY(c, cudaStreamSynchronize(c->copy_out), "cudaStreamSynchronize");
     CU_TRY(c, cudaStreamSynchronize(s), "cudaStreamSynchronize");

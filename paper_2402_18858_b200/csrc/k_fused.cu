@@ -20,8 +20,6 @@
 // `if (lane == 0)` branch ptxas cannot use the uniform datapath and spends ~20 vector instructions + R2UR
 // per MMA, which made ONE thread the bottleneck of the first version of this kernel (465 SASS instructions
 // per 64-column chunk, ~3000 clk against 800 clk of MMA work; profiles/r01_fused_l1l2_v1.md).
-#include <cstdlib>
-#include <cstring>
 #include "common.cuh"
 #include "post.cuh"
 #include "ptx.cuh"
@@ -38,7 +36,6 @@ constexpr int kL1Slots = 3;
 constexpr int kAccCols = 416;    // TMEM columns of the layer-2 accumulator (max pass width)
 constexpr int kL1Col = kAccCols; // L1 slots live in columns 416..511
 constexpr int kFusedThreads = 512;
-constexpr int kSplitThreads = 544;  // k_fused_split: + one forwarder warp
 
 constexpr uint32_t kW2StageBytes = kAccCols * 128;  // 53,248
 constexpr uint32_t kW1StageBytes = kFK * 128;       // 8,192
@@ -58,7 +55,7 @@ enum {
     bW2Full = 0, bW2Empty = bW2Full + kW2Stages, bW1Full = bW2Empty + kW2Stages, bW1Empty = bW1Full + kW1Stages,
     bAFull = bW1Empty + kW1Stages, bAEmpty = bAFull + kAStages, bL1Full = bAEmpty + kAStages,
     bL1Empty = bL1Full + kL1Slots, bZFull = bL1Empty + kL1Slots, bZEmpty = bZFull + 2, bAccFull = bZEmpty + 2,
-    bAccEmpty = bAccFull + 1, bAFullR = bAccEmpty + 1 /* k_fused_split: chunks forwarded by the peer */, bCount = bAFullR + kAStages
+    bAccEmpty = bAccFull + 1, bCount = bAccEmpty + 1
 };
 
 struct FusedArgs {
@@ -436,396 +433,9 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
         ptx::tmem_dealloc(tmem_base, 512);
     }
 }
-// ================================================================================================================
-// k_fused_split -- the same job for nets whose layer 2 needs two passes (H2p in (kAccCols, 2 kAccCols]): the two CTAs of
-// a cluster work on the SAME 128-cell tile and split the layer-2 columns: CTA r accumulates columns [r pass_w, ...) over
-// the full K = H1 -- no passes, so h1 is computed once per tile instead of once per pass.  The h1 chunks are split too:
-// chunk g (global chunk counter) is produced by CTA g & 1 (layer-1 MMA, tcgen05.ld, GELU, BF16) into its own A ring and
-// forwarded to the peer's A ring by one bulk copy through distributed shared memory (warp 16).  Per CTA and tile: 25 chunks of layer-2 MMAs
-// (800 clk each), 12-13 chunks of layer-1 MMAs and h1 GELU, ONE accumulator drain -- against 50 + 50 + 2 before.
-//   AFull[s]   own chunks: 8 arrivals from the local producer warps;  AFullR[s]  the peer's chunks: expect_tx + 16 KB
-//              of the peer forwarder's cp.async.bulk.shared::cluster
-//   AEmpty[s]  in each CTA: 2 tcgen05.commit arrivals (own layer-2 issuer + the peer's, multicast): a stage is rewritten
-//              only when BOTH CTAs' MMAs have read it
-// Everything else (weight rings, layer-1 slots, z, accumulator hand-over) is local to a CTA.
-__global__ void __launch_bounds__(kSplitThreads, 1)
-k_fused_split(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__ CUtensorMap tmapW2a,
-              const __grid_constant__ CUtensorMap tmapW2b, const FusedArgs fa) {
-    extern __shared__ unsigned char smem_raw[];
-    unsigned char *smem = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + kOffBar);
-    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(bars + bCount);
-    float *sBias = reinterpret_cast<float *>(smem + kOffBias);
-    const uint32_t sbase = ptx::smem_u32(smem);
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-
-    int64_t rows = fa.rows;
-    if (fa.n_active) {
-        int64_t r = (int64_t)*fa.n_active - fa.c0;
-        rows = r < 0 ? 0 : (r < rows ? r : rows);
-    }
-    const int n_tiles = (int)((rows + kFM - 1) / kFM);
-    const uint32_t crank = ptx::cluster_ctarank();
-    const uint32_t peer = crank ^ 1u;
-    const int pair = (int)blockIdx.x >> 1, n_pairs = (int)gridDim.x >> 1;
-    const int my_tiles = n_tiles > pair ? (n_tiles - pair + n_pairs - 1) / n_pairs : 0;  // the same for both CTAs
-    const int n_chunks = fa.H1 / kFK;
-    const int total = my_tiles * n_chunks;          // global chunk counter g = it * n_chunks + c; owner = g & 1
-    const int col0 = (int)crank * fa.pass_w;        // first layer-2 column of this CTA
-    int my_w = fa.H2p - col0;
-    my_w = my_w < fa.pass_w ? my_w : fa.pass_w;
-
-    if (threadIdx.x == 0) {
-        for (int i = 0; i < kW2Stages; ++i) { ptx::mbar_init(&bars[bW2Full + i], 1); ptx::mbar_init(&bars[bW2Empty + i], 1); }
-        for (int i = 0; i < kW1Stages; ++i) { ptx::mbar_init(&bars[bW1Full + i], 1); ptx::mbar_init(&bars[bW1Empty + i], 1); }
-        for (int i = 0; i < kAStages; ++i) {
-            ptx::mbar_init(&bars[bAFull + i], 8);    // own chunks: the 8 producer warps
-            ptx::mbar_init(&bars[bAFullR + i], 1);   // the peer's chunks: its forwarder's expect_tx + 16 KB of bulk copy
-            ptx::mbar_init(&bars[bAEmpty + i], 2);
-        }
-        for (int i = 0; i < kL1Slots; ++i) { ptx::mbar_init(&bars[bL1Full + i], 1); ptx::mbar_init(&bars[bL1Empty + i], 4); }
-        for (int i = 0; i < 2; ++i) { ptx::mbar_init(&bars[bZFull + i], 1); ptx::mbar_init(&bars[bZEmpty + i], 1); }
-        ptx::mbar_init(&bars[bAccFull], 1);
-        ptx::mbar_init(&bars[bAccEmpty], 4);
-        ptx::fence_mbar_init();
-    }
-    if (warp == 0 && lane == 0) {
-        ptx::prefetch_tensormap(&tmapW1);
-        ptx::prefetch_tensormap(&tmapW2a);
-        ptx::prefetch_tensormap(&tmapW2b);
-    }
-    if (warp == 1) {
-        ptx::tmem_alloc(tmem_slot, 512);
-        ptx::tmem_relinquish();
-    }
-    for (int i = threadIdx.x; i < fa.H2p && i < (int)(kBias2Bytes / 4); i += kFusedThreads) sBias[i] = fa.bias2[i];
-    ptx::tc_fence_before_sync();
-    __syncthreads();
-    ptx::cluster_sync_all();  // the peer's barriers are initialised before anything of ours can reach them
-    ptx::tc_fence_after_sync();
-    const uint32_t tmem_base = *tmem_slot;
-    const uint64_t desc0 = ptx::umma_desc_sw128_kmajor(sbase);
-
-    if (warp == 0) {
-        // ================================================================ TMA: W2 rows of this CTA for every chunk, W1 rows of its own chunks
-        if (lane == 0) {
-            const uint32_t w2_bytes = (uint32_t)(fa.n0 + fa.n1) * 128u;
-            const int h0 = fa.n0 / 2, h1 = fa.n1 / 2;  // the tensor maps hold half boxes (shared with k_fused_l1l2)
-            Ring w1, w2;
-            for (int i = 0; i < total + 2; ++i) {
-                if (i < total && (uint32_t)(i & 1) == crank) {
-                    const int c = i % n_chunks;
-                    ptx::mbar_wait(&bars[bW1Empty + w1.st], w1.ph ^ 1u);
-                    ptx::mbar_arrive_expect_tx(&bars[bW1Full + w1.st], kW1StageBytes);
-                    unsigned char *d1 = smem + kOffW1 + w1.st * kW1StageBytes;
-                    ptx::tma_load_2d(&tmapW1, &bars[bW1Full + w1.st], d1, 0, c * kFK);
-                    ptx::tma_load_2d(&tmapW1, &bars[bW1Full + w1.st], d1 + kW1StageBytes / 2, 0, c * kFK + kFK / 2);
-                    w1.next(kW1Stages);
-                }
-                if (i >= 2) {
-                    const int c = (i - 2) % n_chunks;
-                    ptx::mbar_wait(&bars[bW2Empty + w2.st], w2.ph ^ 1u);
-                    ptx::mbar_arrive_expect_tx(&bars[bW2Full + w2.st], w2_bytes);
-                    unsigned char *dst = smem + kOffW2 + w2.st * kW2StageBytes;
-                    ptx::tma_load_2d(&tmapW2a, &bars[bW2Full + w2.st], dst, c * kFK, col0);
-                    ptx::tma_load_2d(&tmapW2a, &bars[bW2Full + w2.st], dst + (size_t)h0 * 128, c * kFK, col0 + h0);
-                    if (fa.n1 > 0) {
-                        ptx::tma_load_2d(&tmapW2b, &bars[bW2Full + w2.st], dst + (size_t)fa.n0 * 128, c * kFK, col0 + fa.n0);
-                        ptx::tma_load_2d(&tmapW2b, &bars[bW2Full + w2.st], dst + (size_t)(fa.n0 + h1) * 128, c * kFK,
-                                         col0 + fa.n0 + h1);
-                    }
-                    w2.next(kW2Stages);
-                }
-            }
-        }
-    } else if (warp == 1) {
-        // ================================================================ layer-2 MMA issuer (whole warp, uniform)
-        const uint32_t idesc_n0 = ptx::umma_idesc_bf16_f32(kFM, (uint32_t)fa.n0);
-        const uint32_t idesc_n1 = ptx::umma_idesc_bf16_f32(kFM, (uint32_t)(fa.n1 > 0 ? fa.n1 : 16));
-        const uint64_t b1_off = (uint64_t)((uint32_t)fa.n0 * 128u >> 4);
-        Ring a, w2;
-        uint32_t acc_ph = 0, own_ph = 0, rem_ph = 0;  // per-stage phase bits of AFull / AFullR
-        for (int it = 0; it < my_tiles; ++it) {
-            ptx::mbar_wait(&bars[bAccEmpty], acc_ph ^ 1u);
-            ptx::tc_fence_after_sync();
-            for (int c = 0; c < n_chunks; ++c) {
-                ptx::mbar_wait(&bars[bW2Full + w2.st], w2.ph);
-                {   // own chunks complete AFull (local producers), the peer's chunks AFullR (its forwarder's bulk copy)
-                    const uint32_t bit = 1u << a.st;
-                    if ((uint32_t)((it * n_chunks + c) & 1) == crank) {
-                        ptx::mbar_wait(&bars[bAFull + a.st], (own_ph & bit) ? 1u : 0u);
-                        own_ph ^= bit;
-                    } else {
-                        ptx::mbar_wait_cluster(&bars[bAFullR + a.st], (rem_ph & bit) ? 1u : 0u);
-                        rem_ph ^= bit;
-                    }
-                }
-                ptx::tc_fence_after_sync();
-                const uint64_t da = desc0 + (uint64_t)((kOffA + a.st * kAStageBytes) >> 4);
-                const uint64_t db = desc0 + (uint64_t)((kOffW2 + w2.st * kW2StageBytes) >> 4);
-                if (ptx::elect_one()) {
-#pragma unroll
-                    for (int k = 0; k < kFK / 16; ++k) {
-                        const uint32_t accum = (c | k) ? 1u : 0u;
-                        ptx::umma_bf16_ss(tmem_base, da + 2 * k, db + 2 * k, idesc_n0, accum);
-                        if (fa.n1 > 0)
-                            ptx::umma_bf16_ss(tmem_base + (uint32_t)fa.n0, da + 2 * k, db + b1_off + 2 * k, idesc_n1, accum);
-                    }
-                    ptx::umma_commit_multicast(&bars[bAEmpty + a.st], 3);  // both CTAs' producers wait for both readers
-                    ptx::umma_commit(&bars[bW2Empty + w2.st]);
-                    if (c == n_chunks - 1) ptx::umma_commit(&bars[bAccFull]);
-                }
-                __syncwarp();
-                a.next(kAStages);
-                w2.next(kW2Stages);
-            }
-            acc_ph ^= 1u;
-        }
-    } else if (warp == 2) {
-        // ================================================================ layer-1 MMA issuer: the chunks this CTA owns
-        const uint32_t idesc_l1 = ptx::umma_idesc_bf16_f32(kFM, kSub);
-        Ring w1, slot;
-        int g = 0;
-        for (int it = 0; it < my_tiles; ++it) {
-            const uint32_t zb = (uint32_t)it & 1u;
-            ptx::mbar_wait(&bars[bZFull + zb], ((uint32_t)it >> 1) & 1u);
-            ptx::tc_fence_after_sync();
-            const uint64_t dz = desc0 + (uint64_t)((kOffZ + zb * kZBytes) >> 4);
-            for (int c = 0; c < n_chunks; ++c, ++g) {
-                if ((uint32_t)(g & 1) != crank) continue;
-                ptx::mbar_wait(&bars[bW1Full + w1.st], w1.ph);
-                const uint64_t dw = desc0 + (uint64_t)((kOffW1 + w1.st * kW1StageBytes) >> 4);
-#pragma unroll
-                for (int s = 0; s < 2; ++s) {
-                    ptx::mbar_wait(&bars[bL1Empty + slot.st], slot.ph ^ 1u);
-                    ptx::tc_fence_after_sync();
-                    const uint32_t d_tmem = tmem_base + kL1Col + slot.st * kSub;
-                    const uint64_t dws = dw + (uint64_t)(s * ((kSub * 128) >> 4));
-                    if (ptx::elect_one()) {
-                        for (int k = 0; k < fa.Kz; ++k)
-                            ptx::umma_bf16_ss(d_tmem, dz + 2 * k, dws + 2 * k, idesc_l1, k ? 1u : 0u);
-                        ptx::umma_commit(&bars[bL1Full + slot.st]);
-                    }
-                    __syncwarp();
-                    slot.next(kL1Slots);
-                }
-                if (ptx::elect_one()) ptx::umma_commit(&bars[bW1Empty + w1.st]);
-                __syncwarp();
-                w1.next(kW1Stages);
-            }
-            if (ptx::elect_one()) ptx::umma_commit(&bars[bZEmpty + zb]);
-            __syncwarp();
-        }
-    } else if (warp == 3) {
-        // ================================================================ z builder (32 threads, 4 cells each)
-        const int D = fa.D;
-        const int n_units = 2 * fa.Kz;  // 16-byte units (8 features) that carry data
-        for (int it = 0; it < my_tiles; ++it) {
-            const int tile = pair + it * n_pairs;  // both CTAs of the pair build the z tile of the same cells
-            const int zb = it & 1;
-            ptx::mbar_wait(&bars[bZEmpty + zb], ((uint32_t)(it >> 1) & 1u) ^ 1u);
-            const uint32_t z_addr = sbase + kOffZ + zb * kZBytes;
-            // 4 rows per lane (rr = lane + 32 q).  Loads first, arithmetic after: the 32 independent loads of a
-            // unit (8 features x 4 rows) are in flight together -- one memory latency per unit instead of one per
-            // load (the first version waited for every load in turn and needed ~100k clk per tile)
-            int64_t g4[4];
-            bool ok4[4];
-#pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                const int64_t i = (int64_t)tile * kFM + lane + 32 * q;
-                ok4[q] = i < rows;
-                int64_t g = fa.c0 + i;
-                if (fa.idx) g = ok4[q] ? (int64_t)fa.idx[g] : 0;
-                g4[q] = ok4[q] ? g : 0;
-            }
-#pragma unroll 1
-            for (int u = 0; u < 8; ++u) {
-                float x[4][8];
-                if (u < n_units) {
-#pragma unroll
-                    for (int f = 0; f < 8; ++f) {
-                        const int j = u * 8 + f;
-                        const float *src = j == 0 ? fa.T : (j == 1 ? fa.p : fa.Y + (int64_t)(j - 2) * fa.n);
-#pragma unroll
-                        for (int q = 0; q < 4; ++q) x[q][f] = (j < D && ok4[q]) ? src[g4[q]] : 0.f;
-                    }
-#pragma unroll
-                    for (int f = 0; f < 8; ++f) {
-                        const int j = u * 8 + f;
-                        const float mu = j < D ? fa.pre.mean[j] : 0.f, is = j < D ? fa.pre.inv_std[j] : 0.f;
-#pragma unroll
-                        for (int q = 0; q < 4; ++q) {
-                            float t = x[q][f];
-                            if (j >= 2 && j < D) {
-                                // z is rounded to BF16 (2^-9): the approximate lg2 / ex2 pair (2^-22) is ample here;
-                                // Y = 0 still maps to exactly -1/lambda (R1, R2)
-                                const float Yc = fmaxf(t, 0.f);
-                                if (fa.pre.lambda_zero) t = logf(Yc);
-                                else {
-                                    const float uu = Yc > 0.f ? ptx::ex2_approx(fa.pre.lambda * ptx::lg2_approx(Yc)) : 0.f;
-                                    t = (uu - 1.f) * fa.pre.inv_lambda;
-                                }
-                            }
-                            t = (t - mu) * is;
-                            if (j >= D && j < D + 2) t = 1.f;  // multiplies the hi / lo halves of b1 in W1 columns D, D+1
-                            x[q][f] = ok4[q] ? t : 0.f;
-                        }
-                    }
-                } else {
-#pragma unroll
-                    for (int q = 0; q < 4; ++q)
-#pragma unroll
-                        for (int f = 0; f < 8; ++f) x[q][f] = 0.f;
-                }
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    const int rr = lane + 32 * q;
-                    ptx::st_shared_v4(z_addr + (uint32_t)rr * 128u + (uint32_t)((u ^ (rr & 7)) << 4),
-                                      ptx::pack_bf16x2(x[q][0], x[q][1]), ptx::pack_bf16x2(x[q][2], x[q][3]),
-                                      ptx::pack_bf16x2(x[q][4], x[q][5]), ptx::pack_bf16x2(x[q][6], x[q][7]));
-                }
-            }
-            ptx::fence_proxy_async_smem();
-            __syncwarp();
-            if (lane == 0) ptx::mbar_arrive(&bars[bZFull + zb]);
-        }
-    } else if (warp < 12) {
-        // ================================================================ h1 producers (warps 4..11): the chunks this CTA owns
-        const int q = warp & 3;             // TMEM lane quarter
-        const int set = (warp - 4) >> 2;    // which 32-column half of a 64-column chunk
-        const int r = q * 32 + lane;        // row of the tile
-        const uint32_t lane_addr = tmem_base + ((uint32_t)(q * 32) << 16) + kL1Col;
-        const uint32_t swz = (uint32_t)(r & 7);
-        const uint32_t row_off = (uint32_t)r * 128u;
-        uint32_t slot = (uint32_t)set, slot_ph = 0;  // own sub-chunk j = 2 (own chunk ordinal) + set: slot j % 3, phase (j / 3) & 1
-        uint32_t ast = crank % 3, a_ph = 0;          // A stage / phase of global chunk g = crank, crank + 2, ...
-#pragma unroll 1
-        for (int g = (int)crank; g < total; g += 2) {
-            ptx::mbar_wait(&bars[bL1Full + slot], slot_ph);
-            ptx::tc_fence_after_sync();
-            uint32_t v[32];
-            ptx::tmem_ld32(lane_addr + slot * kSub, v);
-            ptx::tmem_ld_wait();
-            ptx::tc_fence_before_sync();
-            __syncwarp();
-            if (lane == 0) ptx::mbar_arrive(&bars[bL1Empty + slot]);
-            uint32_t o[16];
-#pragma unroll
-            for (int j = 0; j < 16; ++j) o[j] = ptx::gelu2_pack(__uint_as_float(v[2 * j]), __uint_as_float(v[2 * j + 1]));
-            ptx::mbar_wait_cluster(&bars[bAEmpty + ast], a_ph ^ 1u);
-            const uint32_t off = ast * kAStageBytes + row_off;
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                const uint32_t u = ((((uint32_t)(4 * set + i)) ^ swz) << 4);
-                ptx::st_shared_v4(sbase + kOffA + off + u, o[4 * i], o[4 * i + 1], o[4 * i + 2], o[4 * i + 3]);
-            }
-            ptx::fence_proxy_async_smem();  // the MMA and the forwarder's bulk copy read through the async proxy
-            __syncwarp();
-            if (lane == 0) ptx::mbar_arrive(&bars[bAFull + ast]);
-            ast += 2;  // g += 2
-            if (ast >= 3) {
-                ast -= 3;
-                a_ph ^= 1u;
-            }
-            slot += 2;
-            if (slot >= kL1Slots) {
-                slot -= kL1Slots;
-                slot_ph ^= 1u;
-            }
-        }
-    } else if (warp == 16) {
-        // ================================================================ forwarder: own finished A stages -> the peer's A ring
-        // one bulk copy (async proxy, 16 KB) per own chunk, completing on the peer's AFullR barrier; the producers
-        // then pay no remote stores and no cluster-scope fence (those cost ~3,000 clk per chunk, profiles/)
-        if (lane == 0) {
-            uint32_t own_ph = 0;
-            uint32_t ast = crank % 3;
-            const uint32_t ring_peer = ptx::mapa_u32(sbase + kOffA, peer);
-            const uint32_t full_r_peer = ptx::mapa_u32(ptx::smem_u32(&bars[bAFullR]), peer);
-            for (int g = (int)crank; g < total; g += 2) {
-                const uint32_t bit = 1u << ast;
-                ptx::mbar_wait(&bars[bAFull + ast], (own_ph & bit) ? 1u : 0u);
-                own_ph ^= bit;
-                ptx::mbar_arrive_expect_tx_cluster(full_r_peer + ast * 8u, kAStageBytes);
-                ptx::bulk_copy_to_cluster(ring_peer + ast * kAStageBytes, sbase + kOffA + ast * kAStageBytes, kAStageBytes,
-                                          full_r_peer + ast * 8u);
-                ast += 2;
-                if (ast >= 3) ast -= 3;
-            }
-        }
-    } else {
-        // ================================================================ tile epilogue (warps 12..15): the 400 columns of this CTA
-        const int q = warp & 3;
-        const int r = q * 32 + lane;
-        const uint32_t lane_addr = tmem_base + ((uint32_t)(q * 32) << 16);
-        uint32_t acc_ph = 0;
-        for (int it = 0; it < my_tiles; ++it) {
-            const int tile = pair + it * n_pairs;
-            const int64_t grow = (int64_t)tile * kFM + r;
-            const bool row_ok = grow < rows;
-            {
-                ptx::mbar_wait(&bars[bAccFull], acc_ph);
-                ptx::tc_fence_after_sync();
-                acc_ph ^= 1u;
-                const int col_base = col0;
-                const int cur_w = my_w;
-                __nv_bfloat16 *dst_row = fa.h2 + grow * fa.H2p + col_base;
-#pragma unroll 1
-                for (int cc = 0; cc < cur_w; cc += 32) {
-                    const bool full = cc + 32 <= cur_w;  // widths are multiples of 16: the tail piece has 16 columns
-                    uint32_t v[32];
-                    if (full) ptx::tmem_ld32(lane_addr + (uint32_t)cc, v);
-                    else {
-                        uint32_t w[16];
-                        ptx::tmem_ld16(lane_addr + (uint32_t)cc, w);
-#pragma unroll
-                        for (int j = 0; j < 16; ++j) v[j] = w[j];
-#pragma unroll
-                        for (int j = 16; j < 32; ++j) v[j] = 0u;
-                    }
-                    ptx::tmem_ld_wait();
-                    if (cc + 32 >= cur_w) {
-                        // last accumulator read of this warp: hand the accumulator back to the MMA warp
-                        ptx::tc_fence_before_sync();
-                        __syncwarp();
-                        if (lane == 0) ptx::mbar_arrive(&bars[bAccEmpty]);
-                    }
-                    const float4 *b4 = reinterpret_cast<const float4 *>(sBias + col_base + cc);
-                    uint32_t o[16];
-#pragma unroll
-                    for (int j = 0; j < 8; ++j) {
-                        const float4 b = (full || j < 4) ? b4[j] : make_float4(0.f, 0.f, 0.f, 0.f);
-                        o[2 * j] = ptx::gelu2_pack(__uint_as_float(v[4 * j]) + b.x, __uint_as_float(v[4 * j + 1]) + b.y);
-                        o[2 * j + 1] = ptx::gelu2_pack(__uint_as_float(v[4 * j + 2]) + b.z, __uint_as_float(v[4 * j + 3]) + b.w);
-                    }
-                    if (row_ok) {
-                        uint4 *dst = reinterpret_cast<uint4 *>(dst_row + cc);
-                        dst[0] = make_uint4(o[0], o[1], o[2], o[3]);
-                        dst[1] = make_uint4(o[4], o[5], o[6], o[7]);
-                        if (full) {
-                            dst[2] = make_uint4(o[8], o[9], o[10], o[11]);
-                            dst[3] = make_uint4(o[12], o[13], o[14], o[15]);
-                        }
-                    }
-                }
-            }
-        }
-    }
-
-    ptx::tc_fence_before_sync();
-    __syncthreads();
-    ptx::cluster_sync_all();  // no CTA leaves while its peer may still write into it or signal its barriers
-    if (warp == 1) {
-        ptx::tc_fence_after_sync();
-        ptx::tmem_dealloc(tmem_base, 512);
-    }
-}
-
 // ---------------------------------------------------------------- host side
 cudaError_t fused_setup(Ctx *c) {
     (void)c;
-    cudaError_t e = cudaFuncSetAttribute(k_fused_split, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFusedSmem);
-    if (e != cudaSuccess) return e;
     return cudaFuncSetAttribute(k_fused_l1l2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFusedSmem);
 }
 
@@ -887,16 +497,6 @@ cudaError_t launch_fused_l1l2(Ctx *c, int64_t n, int64_t c0, int64_t cn, const f
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    // EXPERIMENTAL (GPUANN_FUSED=split): correct, but 2.92 ms against 2.70 ms per 1 M cells -- the 16 KB per chunk that the
-    // pair exchanges through distributed shared memory is the bound (profiles/r01_fused_l1l2.md)
-    static const bool split = [] { const char *e = std::getenv("GPUANN_FUSED"); return e && std::strcmp(e, "split") == 0; }();
-    if (fn.n_pass == 2 && split) {
-        // two CTAs per tile: as many clusters as there are tiles, at most one per pair of SMs
-        int pairs = (int)(tiles < c->sm_count / 2 ? tiles : c->sm_count / 2);
-        cfg.gridDim = dim3((unsigned)(2 * pairs));
-        cfg.blockDim = dim3(kSplitThreads);
-        return cudaLaunchKernelEx(&cfg, k_fused_split, fn.tmapW1, fn.tmapW2a, fn.tmapW2b, fa);
-    }
     return cudaLaunchKernelEx(&cfg, k_fused_l1l2, fn.tmapW1, fn.tmapW2a, fn.tmapW2b, fa);
 }
 

@@ -30,13 +30,6 @@ constexpr size_t kRegion = (size_t)kWideStages * (kABytes + kBBytesWide) > (size
                                : (size_t)kStages * (kABytes + kBBytesMax);
 constexpr size_t kGemmSmem = 1024 /*align slack*/ + kRegion + 256 + kBiasMax * 4;
 
-// GELU in the tanh form, tanh.approx.f32 (R5: any evaluation inside the BF16 tolerances)
-__device__ __forceinline__ float gelu_tanh(float v) {
-    const float u = v * (0.7978845608028654f + 0.0356774081363001f * v * v);
-    const float hv = 0.5f * v;
-    return fmaf(hv, ptx::tanh_approx(u), hv);
-}
-
 struct GemmArgs {
     int Kp, Np, N;          // padded K, padded N, true N
     int n_tile, tiles_n;

@@ -4,7 +4,7 @@ oracle, run the CUDA path through the C ABI (ctypes binding) and the oracle on t
 Tolerances (BASELINE.json north_star):
   FP32 path: |Y - Y_ref| <= 1e-5 |Y_ref| + 1e-10, max |T - T_ref| <= 1e-3 K
   BF16 path: per output column ||o - o_ref||_2 <= 2e-2 ||o_ref||_2 and max|o - o_ref| <= 2e-2 max|o_ref|,
-             max |T - T_ref| <= 0.5 K
+             max |T - T_ref| <= 0.5 K, |Y - Y_ref| <= 2e-3 |Y_ref| + 1e-10 (R18)
   both:      max |sum_k Y_new - 1| <= 1e-6 (FP64 sum of the stored FP32 values)
 """
 from __future__ import annotations
@@ -28,10 +28,14 @@ class Prepared:
     model: oracle.OracleModel
 
 
-def prepare(cfg: I.Config, n: Optional[int] = None, seed: Optional[int] = None, **over) -> Prepared:
+def prepare(cfg: I.Config, n: Optional[int] = None, seed: Optional[int] = None, mutate=None, **over) -> Prepared:
+    """`mutate(prob)` may edit the drawn problem in place (state, thermo, out_mean, ...) before the derived inputs
+    h (G5) and mu_in / sigma_in (G4) are computed from it."""
     # tiny batches take their normalisation statistics from a 4,096-cell batch of the same seed, then keep n cells
     n_gen = None if n is None else max(int(n), 4096)
     prob = I.make_problem(cfg, n=n_gen, seed=seed)
+    if mutate is not None:
+        mutate(prob)
     st, th = prob.state, prob.thermo
     mean, std = oracle.input_moments(st.T, st.p, st.Y, cfg.lam)                                       # G4
     if n is not None and n_gen != n:
@@ -161,3 +165,47 @@ def check_T_bf16(g: GpuResult, ref, mask=None):
     m = dT.max() if dT.size else 0.0
     assert m <= 0.5, f"T_new: max |dT| = {m:.3e} K > 0.5 K"
     return m
+
+
+def check_Y_bf16(g: GpuResult, ref, mask=None, lam: float = 0.1):
+    """Element-wise Y_new on the BF16 path (R18):
+        |Y - Y_ref| <= 2e-3 max(1, 0.19 / Y_ref^lambda) |Y_ref| + 1e-10.
+    The raw-output error propagates as dY/Y = d(dy) / Y^lambda with d(dy) = dt sigma_out d(o); at the configs'
+    sigma_out dt <= 2e-2 and |d(o)| <~ 1e-2 that is <= 1.1e-3 wherever Y^lambda >= 0.19.  For lambda = 0.1 (all five
+    configs) Y^lambda < 0.19 only below Y = 6e-8, where the absolute floor is the larger term, so the gate IS
+    2e-3 |Y_ref| + 1e-10 there; for another lambda (the branch tests) the factor widens it by the same sensitivity.
+    SURVEY.md Appendix A measured <= 2e-4 relative."""
+    sel = slice(None) if mask is None else mask
+    Yg, Yr = g.Y_new.astype(np.float64)[:, sel], ref.Y_new[:, sel]
+    err = np.abs(Yg - Yr)
+    with np.errstate(divide="ignore"):
+        sens = np.maximum(1.0, 0.19 / np.power(np.abs(Yr), lam)) if lam > 0 else 1.0
+    sens = np.where(np.isfinite(sens), sens, 1.0)
+    tol = 2e-3 * sens * np.abs(Yr) + 1e-10
+    worst = (err / tol).max() if err.size else 0.0
+    assert worst <= 1.0, f"Y_new (BF16 path): max err/tol = {worst:.3f} (tol = 2e-3 s |Y| + 1e-10)"
+    return worst
+
+
+def check_all_bf16(g: GpuResult, ref, mask=None, raw_ref=None, lam: float = 0.1):
+    """Every BF16-path gate at once; returns a dict of the worst figures."""
+    l2, mx = check_raw_bf16(g.o_raw, (ref if raw_ref is None else raw_ref).o_raw)
+    return {"raw_l2": l2, "raw_max": mx, "dT": check_T_bf16(g, ref, mask), "Y": check_Y_bf16(g, ref, mask, lam),
+            "sumY": check_sumY(g.Y_new, mask)}
+
+
+def sample_indices(n, rng, extra, pool=None):
+    """SURVEY.md 8(d) subset S: first 4,096, last 4,096 and `extra` seed-drawn cells (of `pool` if given)."""
+    pool = np.arange(n) if pool is None else np.asarray(pool)
+    head, tail = pool[:4096], pool[-4096:]
+    mid = rng.choice(pool, size=min(extra, pool.size), replace=False)
+    return np.unique(np.concatenate([head, tail, mid]))
+
+
+def subset(pr: Prepared, g: GpuResult, idx):
+    """(oracle result, GPU result) restricted to the cells idx -- the oracle computes only those cells."""
+    st = pr.prob.state
+    ref = run_oracle(pr, T=st.T[idx], p=st.p[idx], Y=np.ascontiguousarray(st.Y[:, idx]), h=pr.h[idx])
+    sub = GpuResult(g.T_new[idx], np.ascontiguousarray(g.Y_new[:, idx]),
+                    None if g.o_raw is None else np.ascontiguousarray(g.o_raw[:, idx]), g.stats)
+    return ref, sub

@@ -13,7 +13,7 @@ from pathlib import Path
 PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libgpuann.so"
-SOURCES = ["api.cu", "k_aux.cu", "k_fp32.cu", "k_gemm.cu", "k_fused.cu"]
+SOURCES = ["api.cu", "k_aux.cu", "k_fp32.cu", "k_gemm.cu", "k_fused.cu", "k_tail.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-std=c++17", "-O3", "-lineinfo",

@@ -69,6 +69,7 @@ void free_net(Ctx *c) {
     }
     cudaFree(c->fused.W1p);
     c->fused = FusedNet{};
+    c->tail.on = false;
     cudaFree(c->act[0]);
     cudaFree(c->act[1]);
     cudaFree(c->o_buf);
@@ -146,6 +147,7 @@ int gpuann_create(const gpuann_params *params, gpuann_ctx **out) {
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->own_stream, cudaStreamNonBlocking);
     if (e == cudaSuccess && prm.precision == GPUANN_PRECISION_BF16) e = gemm_setup(c);
     if (e == cudaSuccess && prm.precision == GPUANN_PRECISION_BF16) e = fused_setup(c);
+    if (e == cudaSuccess && prm.precision == GPUANN_PRECISION_BF16) e = tail_setup(c);
     if (e != cudaSuccess) {
         int rc = fail_cuda(nullptr, e, "gpuann_create");
         gpuann_destroy(c);
@@ -257,6 +259,10 @@ int gpuann_load_net(gpuann_ctx *c, int n_species, int n_layers, const int *sizes
     // variant: "bf16-fused" (S1 + S2 + layers 1-2 in one kernel, k_fused.cu) when the shapes allow it, else
     // "bf16-layerwise"
     const bool fused = n_layers >= 3 && fused_supported(sizes[0], sizes[1], pad16(sizes[2]));
+    // "+tail": the last two layers and the update S4-S8 in one kernel (k_tail.cu); needs a layer in front of them
+    // (the fused kernel or a GEMM) that leaves their input in an activation buffer
+    const bool tail = n_layers >= (fused ? 4 : 2) &&
+                      tail_supported(pad16(sizes[n_layers - 2]), pad16(sizes[n_layers - 1]), n_species);
     int64_t chunk = c->prm.chunk_cells > 0 ? c->prm.chunk_cells : (int64_t)c->sm_count * 128 * (fused ? 56 : 1);
     chunk = (chunk + 127) / 128 * 128;
     c->chunk = chunk;
@@ -323,21 +329,53 @@ int gpuann_load_net(gpuann_ctx *c, int n_species, int n_layers, const int *sizes
         mac += (int64_t)fn.n_pass * H1 * Kz16 - (int64_t)c->lay[0].Kp * c->lay[0].Np;
         mac += (int64_t)H1 * ((int64_t)fn.n_pass * fn.pass_w - l2.Np);
     }
+    // activation scratch: ping-pong buffers [chunk][maxKp]; with the fused kernel in front and the tail kernel behind
+    // only ONE of them is ever used (h2), and the raw output never leaves the SM
     c->act_elems = (size_t)chunk * (size_t)maxKp;
-    for (int b = 0; b < 2; ++b) {
+    const bool one_buffer = fused && tail && n_layers == 4;
+    for (int b = 0; b < (one_buffer ? 1 : 2); ++b) {
         CU_TRY(c, cudaMalloc(&c->act[b], c->act_elems * sizeof(__nv_bfloat16)), "cudaMalloc(activations)");
         CU_TRY(c, cudaMemset(c->act[b], 0, c->act_elems * sizeof(__nv_bfloat16)), "cudaMemset(activations)");
     }
-    CU_TRY(c, cudaMalloc(&c->o_buf, (size_t)n_species * chunk * sizeof(float)), "cudaMalloc(o_buf)");
-    CU_TRY(c, cudaMemset(c->o_buf, 0, (size_t)n_species * chunk * sizeof(float)), "cudaMemset(o_buf)");
+    if (!tail) {
+        CU_TRY(c, cudaMalloc(&c->o_buf, (size_t)n_species * chunk * sizeof(float)), "cudaMalloc(o_buf)");
+        CU_TRY(c, cudaMemset(c->o_buf, 0, (size_t)n_species * chunk * sizeof(float)), "cudaMemset(o_buf)");
+    }
     for (int l = fused ? 2 : 0; l < n_layers; ++l) {
         LayerBf16 &ly = c->lay[l];
         std::string terr;
         if (!encode_tmap_bf16(&ly.tmapA, c->act[l & 1], (uint64_t)ly.Kp, (uint64_t)chunk, (uint64_t)ly.Kp * 2, 128, &terr))
             return fail(c, GPUANN_ERR_CUDA, "gpuann_load_net: " + terr);
     }
+    if (tail) {
+        TailNet &tn = c->tail;
+        const LayerBf16 &l3 = c->lay[n_layers - 2], &l4 = c->lay[n_layers - 1];
+        TailArgs &ta = tn.args;
+        ta.Ns = n_species;
+        ta.Np = l4.Np;
+        ta.K3p = l3.Kp;
+        ta.H3p = l3.Np;
+        tail_plan(l3.Np, &ta.n0, &ta.n1);
+        ta.bias3 = l3.bias;
+        ta.newton_max_iter = po.newton_max_iter;
+        ta.inv_lambda_int = po.inv_lambda_int;
+        ta.lambda_zero = po.lambda_zero;
+        ta.lambda = pre.lambda;
+        ta.inv_lambda = pre.inv_lambda;
+        ta.newton_tol = po.newton_tol;
+        ta.T_min = po.T_min;
+        ta.T_max = po.T_max;
+        for (int k = 0; k < kTailMaxNs; ++k) ta.b4[k] = k < n_species ? biases[n_layers - 1][k] : 0.f;
+        std::string terr;
+        if (!encode_tmap_bf16(&tn.tmapW3a, l3.W, (uint64_t)l3.Kp, (uint64_t)l3.Np, (uint64_t)l3.Kp * 2, (uint32_t)(ta.n0 / 2), &terr) ||
+            !encode_tmap_bf16(&tn.tmapW3b, l3.W, (uint64_t)l3.Kp, (uint64_t)l3.Np, (uint64_t)l3.Kp * 2,
+                              (uint32_t)(ta.n1 > 0 ? ta.n1 / 2 : 8), &terr) ||
+            !encode_tmap_bf16(&tn.tmapW4, l4.W, (uint64_t)l4.Kp, (uint64_t)l4.Np, (uint64_t)l4.Kp * 2, (uint32_t)l4.Np, &terr))
+            return fail(c, GPUANN_ERR_CUDA, "gpuann_load_net: " + terr);
+        tn.on = true;
+    }
     c->issued_mac_per_cell = mac;
-    c->variant = fused ? "bf16-fused" : "bf16-layerwise";
+    c->variant = fused ? (tail ? "bf16-fused+tail" : "bf16-fused") : (tail ? "bf16-layerwise+tail" : "bf16-layerwise");
     c->net_loaded = true;
     return GPUANN_OK;
 }
@@ -379,6 +417,15 @@ int gpuann_load_thermo(gpuann_ctx *c, int n_species, const double *nasa_lo, cons
         }
         h->T_mid[k] = two ? T_mid[k] : 0.0;
     }
+    {
+        TailArgs &ta = c->tail.args;  // the tail kernel takes the table by value (first kTailMaxNs species)
+        ta.two_ranges = h->two_ranges;
+        for (int k = 0; k < kTailMaxNs && k < n_species; ++k) {
+            std::memcpy(ta.th.cp[k], h->cp[k], sizeof(ta.th.cp[k]));
+            std::memcpy(ta.th.hh[k], h->hh[k], sizeof(ta.th.hh[k]));
+            ta.th.T_mid[k] = h->T_mid[k];
+        }
+    }
     DeviceGuard g(c->device);
     cudaDeviceSynchronize();
     cudaError_t e = cudaMemcpy(c->thermo_dev, h, sizeof(ThermoDev), cudaMemcpyHostToDevice);
@@ -413,9 +460,18 @@ int ensure_compaction_scratch(Ctx *c, int64_t n) {
     return GPUANN_OK;
 }
 
-// S1-S3 of the tensor path for the chunk [c0, c0+cn): z -> layers -> raw output o (FP32, [Ns][stride])
-int forward_chunk_bf16(Ctx *c, int64_t n, int64_t c0, int64_t cn, const float *T, const float *p, const float *Y,
-                       bool use_idx, float *o, int64_t o_stride, cudaStream_t s) {
+// what a pass over one chunk produces: the raw network output (gpuann_debug_forward) or the updated state
+struct ChunkOut {
+    float *o_raw = nullptr;   // raw mode: o_raw[k * o_stride + local cell]
+    int64_t o_stride = 0;
+    float *T = nullptr, *Y = nullptr;  // update mode
+    const float *h = nullptr;
+    double dt = 0.0;
+};
+
+// the tensor path for the chunk [c0, c0+cn): z -> layers -> (raw output | update S4-S8)
+int run_chunk_bf16(Ctx *c, int64_t n, int64_t c0, int64_t cn, const float *T, const float *p, const float *Y, bool use_idx,
+                   const ChunkOut &out, cudaStream_t s) {
     int l0 = 0;
     if (c->fused.on) {
         CU_TRY(c, launch_fused_l1l2(c, n, c0, cn, T, p, Y, use_idx, s), "fused kernel");
@@ -423,14 +479,20 @@ int forward_chunk_bf16(Ctx *c, int64_t n, int64_t c0, int64_t cn, const float *T
     } else {
         CU_TRY(c, launch_pre_bf16(c, n, c0, cn, T, p, Y, use_idx, c->act[0], c->lay[0].Kp, s), "pre kernel");
     }
+    const bool raw = out.o_raw != nullptr;
     for (int l = l0; l < c->L; ++l) {
+        if (c->tail.on && l == c->L - 2) {
+            CU_TRY(c, launch_tail(c, n, c0, cn, out.T, out.Y, out.h, out.dt, out.o_raw, out.o_stride, use_idx, s), "tail kernel");
+            return GPUANN_OK;
+        }
         const bool last = l == c->L - 1;
-        __nv_bfloat16 *out = last ? nullptr : c->act[(l + 1) & 1];
+        __nv_bfloat16 *nxt = last ? nullptr : c->act[(l + 1) & 1];
         CU_TRY(c,
-               launch_layer_bf16(c, l, cn, &c->lay[l].tmapA, out, last ? 0 : c->lay[l + 1].Kp, last ? o : nullptr,
-                                 o_stride, c0, use_idx, s),
+               launch_layer_bf16(c, l, cn, &c->lay[l].tmapA, nxt, last ? 0 : c->lay[l + 1].Kp,
+                                 last ? (raw ? out.o_raw : c->o_buf) : nullptr, raw ? out.o_stride : c->chunk, c0, use_idx, s),
                "layer kernel");
     }
+    if (!raw) CU_TRY(c, launch_post(c, n, c0, cn, out.T, out.Y, out.h, c->o_buf, c->chunk, out.dt, use_idx, s), "update kernel");
     return GPUANN_OK;
 }
 
@@ -442,21 +504,6 @@ int check_step_args(Ctx *c, const char *fn, int64_t n, const void *T, const void
     if (n > 0x7FFFFFFFLL) return fail(c, GPUANN_ERR_UNSUPPORTED, std::string(fn) + ": n_cells >= 2^31");
     if (!c->net_loaded || (need_thermo && !c->thermo_loaded))
         return fail(c, GPUANN_ERR_NOT_READY, std::string(fn) + ": load_net" + (need_thermo ? " and load_thermo" : "") + " first");
-    return GPUANN_OK;
-}
-
-struct PostArgsHost {
-    float *T, *Y;
-    const float *h;
-    double dt;
-};
-
-// one slice [a, a+len) of a device-resident field through the tensor path (no compaction): forward + update
-int step_slice_bf16(Ctx *c, int64_t n, int64_t a, int64_t len, const float *T, const float *p, const float *Y,
-                    const PostArgsHost &pa, cudaStream_t s) {
-    int rc = forward_chunk_bf16(c, n, a, len, T, p, Y, false, c->o_buf, c->chunk, s);
-    if (rc != GPUANN_OK) return rc;
-    CU_TRY(c, launch_post(c, n, a, len, pa.T, pa.Y, pa.h, c->o_buf, c->chunk, pa.dt, false, s), "update kernel");
     return GPUANN_OK;
 }
 
@@ -485,11 +532,15 @@ int gpuann_chem_step(gpuann_ctx *c, int64_t n, float *T, const float *p, float *
     } else {
         c->host_active += n;
     }
+    ChunkOut out;
+    out.T = T;
+    out.Y = Y;
+    out.h = h;
+    out.dt = dt;
     for (int64_t c0 = 0; c0 < n; c0 += c->chunk) {
         const int64_t cn = (n - c0) < c->chunk ? (n - c0) : c->chunk;
-        rc = forward_chunk_bf16(c, n, c0, cn, T, p, Y, use_idx, c->o_buf, c->chunk, s);
+        rc = run_chunk_bf16(c, n, c0, cn, T, p, Y, use_idx, out, s);
         if (rc != GPUANN_OK) return rc;
-        CU_TRY(c, launch_post(c, n, c0, cn, T, Y, h, c->o_buf, c->chunk, dt, use_idx, s), "update kernel");
     }
     return GPUANN_OK;
 }
@@ -511,7 +562,10 @@ int gpuann_debug_forward(gpuann_ctx *c, int64_t n, const float *T, const float *
     }
     for (int64_t c0 = 0; c0 < n; c0 += c->chunk) {
         const int64_t cn = (n - c0) < c->chunk ? (n - c0) : c->chunk;
-        rc = forward_chunk_bf16(c, n, c0, cn, T, p, Y, false, o_raw + c0, n, s);
+        ChunkOut out;
+        out.o_raw = o_raw + c0;
+        out.o_stride = n;
+        rc = run_chunk_bf16(c, n, c0, cn, T, p, Y, false, out, s);
         if (rc != GPUANN_OK) return rc;
     }
     return GPUANN_OK;
@@ -600,8 +654,12 @@ int gpuann_chem_step_host(gpuann_ctx *c, int64_t n, float *T, const float *p, fl
         CU_TRY_DRAIN(cudaMemcpy2DAsync(dY + a, pitch, Y + a, pitch, lb, Ns, cudaMemcpyHostToDevice, c->copy_in), "H2D Y");
         CU_TRY_DRAIN(cudaEventRecord(e_in, c->copy_in), "cudaEventRecord");
         CU_TRY_DRAIN(cudaStreamWaitEvent(s, e_in, 0), "cudaStreamWaitEvent");
-        const PostArgsHost pa{dT, dY, dh, dt};
-        rc = step_slice_bf16(c, n, a, len, dT, dp, dY, pa, s);
+        ChunkOut out;
+        out.T = dT;
+        out.Y = dY;
+        out.h = dh;
+        out.dt = dt;
+        rc = run_chunk_bf16(c, n, a, len, dT, dp, dY, false, out, s);
         if (rc != GPUANN_OK) {
             drain();
             return rc;
@@ -711,7 +769,7 @@ const char *gpuann_timing_class_name(int cls) {
     static const char *names[kNumKernelClasses] = {"compact",      "pre_boxcox_norm", "layer0_gemm", "layer1_gemm",
                                                    "layer2_gemm",  "layer3_gemm",     "layer4_gemm", "layer5_gemm",
                                                    "layer6_gemm",  "layer7_gemm",     "post_update_newton",
-                                                   "fp32_fused",   "bf16_fused",      "aux"};
+                                                   "fp32_fused",   "bf16_fused",      "aux",         "bf16_tail"};
     return (cls >= 0 && cls < kNumKernelClasses) ? names[cls] : "";
 }
 

@@ -82,6 +82,39 @@ struct FusedNet {
     int n_pass = 0, pass_w = 0, n0 = 0, n1 = 0;
 };
 
+// tail kernel (k_tail.cu): the last two layers + S4-S8.  TailArgs is the kernel's by-value parameter block: the
+// thermo table and the per-species constants sit in the constant bank, where warp-uniform reads cost nothing.
+constexpr int kTailMaxNs = 48;
+struct TailThermo {
+    double cp[kTailMaxNs][2][5];  // as ThermoDev
+    double hh[kTailMaxNs][2][6];
+    double T_mid[kTailMaxNs];
+};
+struct TailArgs {
+    int64_t n, c0, rows;
+    const int32_t *n_active, *idx;
+    float *T, *Y;
+    const float *h;
+    float *o_raw;  // != nullptr: forward only, o + b4 -> o_raw[k * o_stride + local cell]
+    int64_t o_stride;
+    int Ns, Np;    // species, padded to 16
+    int K3p, H3p, n0, n1;
+    const float *bias3;
+    int newton_max_iter, inv_lambda_int, lambda_zero, two_ranges;
+    float lambda, inv_lambda;
+    double newton_tol, T_min, T_max;
+    float sA[kTailMaxNs];  // dt sigma_out,k
+    float sC[kTailMaxNs];  // dt (sigma_out,k b4,k + mu_out,k)
+    float b4[kTailMaxNs];
+    Counters *counters;
+    TailThermo th;
+};
+struct TailNet {
+    bool on = false;
+    CUtensorMap tmapW3a{}, tmapW3b{}, tmapW4{};  // W3 half boxes {64, n0/2}, {64, n1/2}; W4 box {64, Np}
+    TailArgs args{};
+};
+
 struct Ctx {
     gpuann_params prm{};
     int device = 0;
@@ -109,6 +142,7 @@ struct Ctx {
     int64_t issued_mac_per_cell = 0;
     const char *variant = "none";
     FusedNet fused;
+    TailNet tail;
 
     // thermo
     bool thermo_loaded = false;
@@ -153,7 +187,8 @@ enum KernelClass {
     kClsFp32 = 11,
     kClsFused = 12,
     kClsAux = 13,
-    kNumKernelClasses = 14
+    kClsTail = 14,
+    kNumKernelClasses = 15
 };
 
 // RAII: counts the launch and, when timing is on, brackets it with two events on the launching stream.
@@ -211,6 +246,13 @@ bool fused_supported(int D, int H1, int H2p);
 void fused_plan(int H2p, int *n_pass, int *pass_w, int *n0, int *n1);
 cudaError_t launch_fused_l1l2(Ctx *c, int64_t n, int64_t c0, int64_t cn, const float *T, const float *p, const float *Y,
                               bool use_idx, cudaStream_t s);
+
+// k_tail.cu
+cudaError_t tail_setup(Ctx *c);
+bool tail_supported(int K3p, int H3p, int Ns);
+void tail_plan(int H3p, int *n0, int *n1);
+cudaError_t launch_tail(Ctx *c, int64_t n, int64_t c0, int64_t cn, float *T, float *Y, const float *h, double dt,
+                        float *o_raw, int64_t o_stride, bool use_idx, cudaStream_t s);
 
 // encodes a 2-D BF16 row-major tensor map {inner = cols, outer = rows}, box {64, box_rows}, 128-byte swizzle
 bool encode_tmap_bf16(CUtensorMap *out, const void *base, uint64_t cols, uint64_t rows, uint64_t row_pitch_bytes,

@@ -1,0 +1,528 @@
+// k_tail.cu -- tensor path, last kernel: the LAST TWO layers of S3 and the whole update S4-S8 in one persistent kernel
+//     h3 = GELU(h2 W3^T + b3)      [128 x H3]   accumulated in TMEM, never leaves the SM
+//     o  = h3 W4^T + b4            [128 x Ns]   accumulated in TMEM
+//     dy = dt (o sigma_out + mu_out);  Y* = F^-1(F(Y) + dy);  Y_new = Y* / sum Y*;  Newton for T_new; store in place
+//                                                                      (PAPER.md:98-103 Eq. 7, :92, :57; R3, R7-R11)
+// Why: the separate layer-3, layer-4 and update kernels moved h3 (0.84 GB at configs[2]) and o through HBM and ran the
+// N = 32 layer-4 GEMM at 7 % of the tensor pipe behind an 80 %-of-HBM stream; here h3 goes TMEM -> registers -> a
+// 16 KB shared-memory chunk -> the layer-4 MMA, and the update runs on four warps in the shadow of the next tile's MMAs.
+//
+// Roles (512 threads, one CTA per SM in clusters of 2, 128-cell tiles walked with stride gridDim.x):
+//   warp 0       TMA: A = h2 tile k-block [128 x 64] (own) + B = W3 k-block [H3p x 64]: each CTA of the pair loads HALF
+//                of B and multicasts it to both (ring of 2); W4 [Np x K4] once, resident
+//   warp 1       layer-3 tcgen05.mma issuer + TMEM owner: acc[0..H3p) += A x B (two MMAs per k-step when H3p > 256)
+//   warp 2       layer-4 tcgen05.mma issuer: o[ob] += h3 chunk (smem) x W4 chunk (smem), two o accumulators
+//   warps 4-11   drain: tcgen05.ld 32 columns of acc -> + b3 -> 2 GELU -> BF16 -> swizzled 64-column h3 chunk (ring of 2)
+//   warps 12-15  update, one thread per cell: state loads (gathered through idx under compaction) issued BEFORE waiting
+//                for o; species update in FP32 (Y^lambda by lg2/ex2, integer power 1/lambda), sum of Y* and the NASA-7
+//                MIXTURE coefficients sum_k Y_k c_kj accumulated in FP64 while the species stream by, then Newton on the
+//                two mixture polynomials in FP64: 11 FMAs per iteration instead of 11 Ns (one-range tables; a two-range
+//                table re-selects per species and iteration).  DESIGN.md "Precision of the scalar math".
+#include "common.cuh"
+#include "ptx.cuh"
+
+namespace gpuann {
+
+constexpr int kTM = 128;            // cells per tile
+constexpr int kTK = 64;             // K elements per smem row (128 B)
+constexpr int kTStages = 2;
+constexpr int kTAccMax = 416;       // TMEM columns of the layer-3 accumulator
+constexpr int kTOCol = 416;         // two o accumulators of kTOStride columns follow
+constexpr int kTOStride = 48;
+constexpr int kTMaxChunks = (kTAccMax + 63) / 64;  // 7
+constexpr int kTailThreads = 512;
+constexpr uint32_t kTABytes = kTM * 128;            // 16,384
+constexpr uint32_t kTBBytes = kTAccMax * 128;       // 53,248
+constexpr uint32_t kTStageBytes = kTABytes + kTBBytes;
+constexpr uint32_t kTH3Bytes = kTM * 128;
+constexpr uint32_t kTW4Bytes = kTMaxChunks * kTailMaxNs * 128;  // 43,008
+constexpr uint32_t kTOffH3 = kTStages * kTStageBytes;
+constexpr uint32_t kTOffW4 = kTOffH3 + 2 * kTH3Bytes;
+constexpr uint32_t kTOffBias = kTOffW4 + kTW4Bytes;
+constexpr uint32_t kTOffBar = kTOffBias + 2048;
+constexpr size_t kTailSmem = 1024 + kTOffBar + 256;
+
+enum {
+    tFull = 0, tEmpty = tFull + kTStages, tW4Full = tEmpty + kTStages, tAccFull, tAccEmpty, tH3Full, tH3Empty = tH3Full + 2,
+    tOFull = tH3Empty + 2, tOEmpty = tOFull + 2, tCount = tOEmpty + 2
+};
+
+struct TRing {
+    uint32_t st = 0, ph = 0;
+    __device__ __forceinline__ void next(uint32_t n) {
+        if (++st == n) {
+            st = 0;
+            ph ^= 1u;
+        }
+    }
+};
+
+__device__ __forceinline__ float powi_f(float x, int n) {
+    float r = 1.f;
+    while (n) {
+        if (n & 1) r *= x;
+        x *= x;
+        n >>= 1;
+    }
+    return r;
+}
+
+__device__ __forceinline__ double horner5(const double *c, double T) {
+    return c[0] + T * (c[1] + T * (c[2] + T * (c[3] + T * c[4])));
+}
+__device__ __forceinline__ double horner6(const double *c, double T) {
+    return c[0] + T * (c[1] + T * (c[2] + T * (c[3] + T * (c[4] + T * c[5]))));
+}
+
+// S4 + S5 for one species in FP32 (R3, R7): Y* = Yc (max(1 + lambda dy / Yc^lambda, 0))^(1/lambda); Yc = 0 (or so small that
+// Yc^lambda flushes to 0): Y* = max(lambda dy, 0)^(1/lambda); lambda = 0: Y* = Yc exp(dy)
+__device__ __forceinline__ float update_species_f32(float yc, float dy, const TailArgs &ta) {
+    if (ta.lambda_zero) return yc * expf(dy);
+    const float u = yc > 0.f ? ptx::ex2_approx(ta.lambda * ptx::lg2_approx(yc)) : 0.f;
+    const float ldy = ta.lambda * dy;
+    const bool pos = u > 0.f;
+    const float base = fmaxf(pos ? 1.f + __fdividef(ldy, u) : ldy, 0.f);
+    float pw;
+    if (ta.inv_lambda_int == 10) {
+        const float b2 = base * base, b4 = b2 * b2;
+        pw = b4 * b4 * b2;
+    } else if (ta.inv_lambda_int > 0) {
+        pw = powi_f(base, ta.inv_lambda_int);
+    } else {
+        pw = powf(base, ta.inv_lambda);
+    }
+    return (pos ? yc : 1.f) * pw;
+}
+
+template <int NSP>
+__global__ void __launch_bounds__(kTailThreads, 1)
+k_tail(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ CUtensorMap tmapW3a,
+       const __grid_constant__ CUtensorMap tmapW3b, const __grid_constant__ CUtensorMap tmapW4,
+       const __grid_constant__ TailArgs ta) {
+    extern __shared__ unsigned char smem_raw[];
+    unsigned char *smem = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + kTOffBar);
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(bars + tCount);
+    float *sBias = reinterpret_cast<float *>(smem + kTOffBias);
+    const uint32_t sbase = ptx::smem_u32(smem);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    int64_t rows = ta.rows;
+    if (ta.n_active) {
+        int64_t r = (int64_t)*ta.n_active - ta.c0;
+        rows = r < 0 ? 0 : (r < rows ? r : rows);
+    }
+    const int n_tiles = (int)((rows + kTM - 1) / kTM);
+    // both CTAs of a pair walk the same number of tiles (they share every W3 stage); the odd one may get an empty tile
+    const uint32_t crank = ptx::cluster_ctarank();
+    const int pair_first = (int)blockIdx.x & ~1;
+    const int my_tiles = n_tiles > pair_first ? (n_tiles - pair_first + (int)gridDim.x - 1) / (int)gridDim.x : 0;
+    const int nkb = (ta.K3p + kTK - 1) / kTK;
+    const int nch = (ta.H3p + 63) / 64;
+
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < kTStages; ++i) { ptx::mbar_init(&bars[tFull + i], 1); ptx::mbar_init(&bars[tEmpty + i], 2); }
+        ptx::mbar_init(&bars[tW4Full], 1);
+        ptx::mbar_init(&bars[tAccFull], 1);
+        ptx::mbar_init(&bars[tAccEmpty], 8);
+        for (int i = 0; i < 2; ++i) {
+            ptx::mbar_init(&bars[tH3Full + i], 8);
+            ptx::mbar_init(&bars[tH3Empty + i], 1);
+            ptx::mbar_init(&bars[tOFull + i], 1);
+            ptx::mbar_init(&bars[tOEmpty + i], 4);
+        }
+        ptx::fence_mbar_init();
+    }
+    if (warp == 0 && lane == 0) {
+        ptx::prefetch_tensormap(&tmapA);
+        ptx::prefetch_tensormap(&tmapW3a);
+        ptx::prefetch_tensormap(&tmapW3b);
+        ptx::prefetch_tensormap(&tmapW4);
+    }
+    if (warp == 1) {
+        ptx::tmem_alloc(tmem_slot, 512);
+        ptx::tmem_relinquish();
+    }
+    for (int i = threadIdx.x; i < ta.H3p && i < kTAccMax; i += kTailThreads) sBias[i] = ta.bias3[i];
+    ptx::tc_fence_before_sync();
+    __syncthreads();
+    ptx::cluster_sync_all();
+    ptx::tc_fence_after_sync();
+    const uint32_t tmem_base = *tmem_slot;
+    const uint64_t desc0 = ptx::umma_desc_sw128_kmajor(sbase);
+
+    if (warp == 0) {
+        // ================================================================ TMA
+        if (lane == 0) {
+            ptx::mbar_arrive_expect_tx(&bars[tW4Full], (uint32_t)(nch * ta.Np * 128));
+            for (int c = 0; c < nch; ++c)
+                ptx::tma_load_2d(&tmapW4, &bars[tW4Full], smem + kTOffW4 + (size_t)c * ta.Np * 128, c * kTK, 0);
+            const uint32_t stage_bytes = kTABytes + (uint32_t)(ta.n0 + ta.n1) * 128u;
+            const int h0 = ta.n0 / 2, h1 = ta.n1 / 2;
+            TRing st;
+            for (int it = 0; it < my_tiles; ++it) {
+                const int tile = (int)blockIdx.x + it * (int)gridDim.x;
+                for (int kb = 0; kb < nkb; ++kb) {
+                    ptx::mbar_wait(&bars[tEmpty + st.st], st.ph ^ 1u);
+                    ptx::mbar_arrive_expect_tx(&bars[tFull + st.st], stage_bytes);
+                    unsigned char *sA = smem + (size_t)st.st * kTStageBytes;
+                    unsigned char *sB = sA + kTABytes;
+                    ptx::tma_load_2d(&tmapA, &bars[tFull + st.st], sA, kb * kTK, tile * kTM);
+                    ptx::tma_load_2d_multicast(&tmapW3a, &bars[tFull + st.st], sB + (size_t)crank * h0 * 128, kb * kTK,
+                                               (int)crank * h0, 3);
+                    if (ta.n1 > 0)
+                        ptx::tma_load_2d_multicast(&tmapW3b, &bars[tFull + st.st],
+                                                   sB + (size_t)ta.n0 * 128 + (size_t)crank * h1 * 128, kb * kTK,
+                                                   ta.n0 + (int)crank * h1, 3);
+                    st.next(kTStages);
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ================================================================ layer-3 MMA issuer (whole warp, uniform)
+        const uint32_t idesc0 = ptx::umma_idesc_bf16_f32(kTM, (uint32_t)ta.n0);
+        const uint32_t idesc1 = ptx::umma_idesc_bf16_f32(kTM, (uint32_t)(ta.n1 > 0 ? ta.n1 : 16));
+        const uint64_t b1_off = (uint64_t)(((uint32_t)ta.n0 * 128u) >> 4);
+        TRing st;
+        uint32_t acc_ph = 0;
+        for (int it = 0; it < my_tiles; ++it) {
+            ptx::mbar_wait(&bars[tAccEmpty], acc_ph ^ 1u);
+            ptx::tc_fence_after_sync();
+            for (int kb = 0; kb < nkb; ++kb) {
+                ptx::mbar_wait(&bars[tFull + st.st], st.ph);
+                ptx::tc_fence_after_sync();
+                const uint64_t da = desc0 + (uint64_t)((st.st * kTStageBytes) >> 4);
+                const uint64_t db = da + (uint64_t)(kTABytes >> 4);
+                const int ksteps = min(kTK / 16, (ta.K3p - kb * kTK) / 16);
+                if (ptx::elect_one()) {
+                    if (ksteps == kTK / 16) {
+#pragma unroll
+                        for (int k = 0; k < kTK / 16; ++k) {
+                            ptx::umma_bf16_ss(tmem_base, da + 2 * k, db + 2 * k, idesc0, (kb | k) ? 1u : 0u);
+                            if (ta.n1 > 0)
+                                ptx::umma_bf16_ss(tmem_base + (uint32_t)ta.n0, da + 2 * k, db + b1_off + 2 * k, idesc1, (kb | k) ? 1u : 0u);
+                        }
+                    } else {
+                        for (int k = 0; k < ksteps; ++k) {
+                            ptx::umma_bf16_ss(tmem_base, da + 2 * k, db + 2 * k, idesc0, (kb | k) ? 1u : 0u);
+                            if (ta.n1 > 0)
+                                ptx::umma_bf16_ss(tmem_base + (uint32_t)ta.n0, da + 2 * k, db + b1_off + 2 * k, idesc1, (kb | k) ? 1u : 0u);
+                        }
+                    }
+                    ptx::umma_commit_multicast(&bars[tEmpty + st.st], 3);
+                    if (kb == nkb - 1) ptx::umma_commit(&bars[tAccFull]);
+                }
+                __syncwarp();
+                st.next(kTStages);
+            }
+            acc_ph ^= 1u;
+        }
+    } else if (warp == 2) {
+        // ================================================================ layer-4 MMA issuer (whole warp, uniform)
+        const uint32_t idesc4 = ptx::umma_idesc_bf16_f32(kTM, (uint32_t)ta.Np);
+        ptx::mbar_wait(&bars[tW4Full], 0);
+        uint32_t seq = 0;
+        for (int it = 0; it < my_tiles; ++it) {
+            const uint32_t ob = (uint32_t)it & 1u, oph = ((uint32_t)it >> 1) & 1u;
+            ptx::mbar_wait(&bars[tOEmpty + ob], oph ^ 1u);
+            ptx::tc_fence_after_sync();
+            const uint32_t d_tmem = tmem_base + kTOCol + ob * kTOStride;
+            for (int c = 0; c < nch; ++c, ++seq) {
+                const uint32_t buf = seq & 1u, ph = (seq >> 1) & 1u;
+                ptx::mbar_wait(&bars[tH3Full + buf], ph);
+                ptx::tc_fence_after_sync();
+                const uint64_t da = desc0 + (uint64_t)((kTOffH3 + buf * kTH3Bytes) >> 4);
+                const uint64_t db = desc0 + (uint64_t)((kTOffW4 + (uint32_t)c * (uint32_t)ta.Np * 128u) >> 4);
+                const int ksteps = min(4, (ta.H3p - c * 64) / 16);
+                if (ptx::elect_one()) {
+                    for (int k = 0; k < ksteps; ++k)
+                        ptx::umma_bf16_ss(d_tmem, da + 2 * k, db + 2 * k, idesc4, (c | k) ? 1u : 0u);
+                    ptx::umma_commit(&bars[tH3Empty + buf]);
+                    if (c == nch - 1) ptx::umma_commit(&bars[tOFull + ob]);
+                }
+                __syncwarp();
+            }
+        }
+    } else if (warp >= 4 && warp < 12) {
+        // ================================================================ drain: acc -> h3 chunks (warps 4..11)
+        const int q = warp & 3;           // TMEM lane quarter
+        const int hsel = (warp - 4) >> 2; // which 32-column half of every 64-column chunk
+        const int r = q * 32 + lane;
+        const uint32_t lane_addr = tmem_base + ((uint32_t)(q * 32) << 16);
+        const uint32_t swz = (uint32_t)(r & 7);
+        const uint32_t row_off = (uint32_t)r * 128u;
+        uint32_t acc_ph = 0, seq = 0;
+        for (int it = 0; it < my_tiles; ++it) {
+            ptx::mbar_wait(&bars[tAccFull], acc_ph);
+            ptx::tc_fence_after_sync();
+            acc_ph ^= 1u;
+#pragma unroll 1
+            for (int c = 0; c < nch; ++c, ++seq) {
+                const int cc = c * 64 + hsel * 32;
+                const int w = ta.H3p - cc;  // >= 32: full piece; 16: half piece; <= 0: none (widths are multiples of 16)
+                uint32_t v[32];
+                if (w >= 32) ptx::tmem_ld32(lane_addr + (uint32_t)cc, v);
+                else if (w > 0) {
+                    uint32_t t[16];
+                    ptx::tmem_ld16(lane_addr + (uint32_t)cc, t);
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) v[j] = t[j];
+#pragma unroll
+                    for (int j = 16; j < 32; ++j) v[j] = 0u;
+                } else {
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) v[j] = 0u;
+                }
+                ptx::tmem_ld_wait();
+                if (c == nch - 1) {  // last accumulator read of this warp in this tile
+                    ptx::tc_fence_before_sync();
+                    __syncwarp();
+                    if (lane == 0) ptx::mbar_arrive(&bars[tAccEmpty]);
+                }
+                uint32_t o[16];
+                if (w > 0) {
+                    const float4 *b4 = reinterpret_cast<const float4 *>(sBias + cc);
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) {
+                        const float4 b = (w >= 32 || j < 4) ? b4[j] : make_float4(0.f, 0.f, 0.f, 0.f);
+                        o[2 * j] = ptx::gelu2_pack(__uint_as_float(v[4 * j]) + b.x, __uint_as_float(v[4 * j + 1]) + b.y);
+                        o[2 * j + 1] = ptx::gelu2_pack(__uint_as_float(v[4 * j + 2]) + b.z, __uint_as_float(v[4 * j + 3]) + b.w);
+                    }
+                }
+                const uint32_t buf = seq & 1u, ph = (seq >> 1) & 1u;
+                ptx::mbar_wait(&bars[tH3Empty + buf], ph ^ 1u);
+                if (w > 0) {
+                    const uint32_t row_addr = sbase + kTOffH3 + buf * kTH3Bytes + row_off;
+#pragma unroll
+                    for (int i = 0; i < 4; ++i)
+                        if (w >= 32 || i < 2)
+                            ptx::st_shared_v4(row_addr + ((((uint32_t)(4 * hsel + i)) ^ swz) << 4), o[4 * i], o[4 * i + 1],
+                                              o[4 * i + 2], o[4 * i + 3]);
+                    ptx::fence_proxy_async_smem();
+                }
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive(&bars[tH3Full + buf]);
+            }
+        }
+    } else if (warp >= 12) {
+        // ================================================================ update S4-S8 (warps 12..15), one thread per cell
+        const int q = warp & 3;
+        const int r = q * 32 + lane;
+        const uint32_t lane_addr = tmem_base + ((uint32_t)(q * 32) << 16) + kTOCol;
+        const int Ns = ta.Ns;
+        unsigned nconv_total = 0, ndeg_total = 0;
+        for (int it = 0; it < my_tiles; ++it) {
+            const int tile = (int)blockIdx.x + it * (int)gridDim.x;
+            const int64_t i = (int64_t)tile * kTM + r;
+            const bool valid = i < rows;
+            int64_t g = ta.c0 + i;
+            if (ta.idx) g = valid ? (int64_t)ta.idx[g] : 0;
+            if (!valid) g = 0;
+            const uint32_t ob = (uint32_t)it & 1u, oph = ((uint32_t)it >> 1) & 1u;
+            const bool fwd_only = ta.o_raw != nullptr;
+            // state loads first: their latency hides behind the wait for o
+            float Yv[NSP];
+            float Tin = 300.f, hin = 0.f;
+            if (!fwd_only) {
+#pragma unroll
+                for (int k = 0; k < NSP; ++k) Yv[k] = (valid && k < Ns) ? ta.Y[(int64_t)k * ta.n + g] : 0.f;
+                if (valid) {
+                    Tin = ta.T[g];
+                    hin = ta.h[g];
+                }
+            }
+            ptx::mbar_wait(&bars[tOFull + ob], oph);
+            ptx::tc_fence_after_sync();
+            double S = 0.0;
+            double Ch[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0}, Cc[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+            for (int pc = 0; pc < NSP / 16; ++pc) {
+                uint32_t ov[16];
+                ptx::tmem_ld16(lane_addr + ob * kTOStride + (uint32_t)(16 * pc), ov);
+                ptx::tmem_ld_wait();
+                if (pc == NSP / 16 - 1) {  // o is in registers: hand the accumulator back to the layer-4 issuer
+                    ptx::tc_fence_before_sync();
+                    __syncwarp();
+                    if (lane == 0) ptx::mbar_arrive(&bars[tOEmpty + ob]);
+                }
+#pragma unroll
+                for (int j = 0; j < 16; ++j) {
+                    const int k = 16 * pc + j;
+                    if (k < Ns) {
+                        const float o = __uint_as_float(ov[j]);
+                        if (fwd_only) {
+                            if (valid) ta.o_raw[(int64_t)k * ta.o_stride + i] = o + ta.b4[k];
+                        } else {
+                            const float ys = update_species_f32(fmaxf(Yv[k], 0.f), fmaf(o, ta.sA[k], ta.sC[k]), ta);
+                            Yv[k] = ys;
+                            const double yd = (double)ys;
+                            S += yd;
+                            if (!ta.two_ranges) {
+#pragma unroll
+                                for (int m = 0; m < 6; ++m) Ch[m] = fma(yd, ta.th.hh[k][0][m], Ch[m]);
+#pragma unroll
+                                for (int m = 0; m < 5; ++m) Cc[m] = fma(yd, ta.th.cp[k][0][m], Cc[m]);
+                            }
+                        }
+                    }
+                }
+            }
+            if (fwd_only) continue;
+            // S6 (R8): divide by the sum; a vanishing sum falls back to max(Y,0)/sum (rare: the inputs are re-read)
+            const bool degenerate = !(S > 0.0);
+            double rS;
+            if (!degenerate) {
+                rS = 1.0 / S;
+            } else {
+                double Sc = 0.0;
+#pragma unroll
+                for (int k = 0; k < NSP; ++k) {
+                    Yv[k] = (valid && k < Ns) ? fmaxf(ta.Y[(int64_t)k * ta.n + g], 0.f) : 0.f;
+                    Sc += (double)Yv[k];
+                }
+                rS = 1.0 / Sc;
+#pragma unroll
+                for (int m = 0; m < 6; ++m) Ch[m] = 0.0;
+#pragma unroll
+                for (int m = 0; m < 5; ++m) Cc[m] = 0.0;
+                if (!ta.two_ranges) {
+#pragma unroll
+                    for (int k = 0; k < NSP; ++k)
+                        if (k < Ns) {
+                            const double yd = (double)Yv[k];
+#pragma unroll
+                            for (int m = 0; m < 6; ++m) Ch[m] = fma(yd, ta.th.hh[k][0][m], Ch[m]);
+#pragma unroll
+                            for (int m = 0; m < 5; ++m) Cc[m] = fma(yd, ta.th.cp[k][0][m], Cc[m]);
+                        }
+                }
+            }
+#pragma unroll
+            for (int m = 0; m < 6; ++m) Ch[m] *= rS;
+#pragma unroll
+            for (int m = 0; m < 5; ++m) Cc[m] *= rS;
+            // S7 (R9-R11): Newton on h(T) = sum_k Y_k h_k(T), FP64
+            double Tn = fmin(fmax((double)Tin, ta.T_min), ta.T_max);
+            bool conv = false;
+            const double hc = (double)hin;
+            for (int itn = 0; itn < ta.newton_max_iter; ++itn) {
+                double f, c;
+                if (!ta.two_ranges) {
+                    f = horner6(Ch, Tn) - hc;
+                    c = horner5(Cc, Tn);
+                } else {
+                    f = 0.0;
+                    c = 0.0;
+#pragma unroll
+                    for (int k = 0; k < NSP; ++k)
+                        if (k < Ns) {
+                            const int rg = !(Tn < ta.th.T_mid[k]) ? 1 : 0;
+                            const double yd = (double)Yv[k] * rS;
+                            f = fma(yd, horner6(ta.th.hh[k][rg], Tn), f);
+                            c = fma(yd, horner5(ta.th.cp[k][rg], Tn), c);
+                        }
+                    f -= hc;
+                }
+                if (!(c > 0.0)) break;  // R10: stop, not converged
+                const double dT = -f / c;
+                Tn = fmin(fmax(Tn + dT, ta.T_min), ta.T_max);
+                if (fabs(dT) < ta.newton_tol) {
+                    conv = true;
+                    break;
+                }
+            }
+            // S8: store in place (skipped / out-of-range cells are never touched)
+            if (valid) {
+#pragma unroll
+                for (int k = 0; k < NSP; ++k)
+                    if (k < Ns) ta.Y[(int64_t)k * ta.n + g] = (float)((double)Yv[k] * rS);
+                ta.T[g] = (float)Tn;
+                if (!conv) ++nconv_total;
+                if (degenerate) ++ndeg_total;
+            }
+        }
+        // statistics: one atomic per warp and counter, only when something happened
+        nconv_total = __reduce_add_sync(0xffffffffu, nconv_total);
+        ndeg_total = __reduce_add_sync(0xffffffffu, ndeg_total);
+        if (lane == 0) {
+            if (nconv_total) atomicAdd(&ta.counters->n_not_converged, (unsigned long long)nconv_total);
+            if (ndeg_total) atomicAdd(&ta.counters->n_degenerate, (unsigned long long)ndeg_total);
+        }
+    }
+
+    ptx::tc_fence_before_sync();
+    __syncthreads();
+    ptx::cluster_sync_all();  // no CTA leaves while its peer may still multicast into it or signal its barriers
+    if (warp == 1) {
+        ptx::tc_fence_after_sync();
+        ptx::tmem_dealloc(tmem_base, 512);
+    }
+}
+
+// ---------------------------------------------------------------- host side
+cudaError_t tail_setup(Ctx *c) {
+    (void)c;
+    cudaError_t e = cudaFuncSetAttribute(k_tail<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTailSmem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_tail<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTailSmem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_tail<48>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTailSmem);
+    return e;
+}
+
+bool tail_supported(int K3p, int H3p, int Ns) {
+    return K3p >= 16 && K3p % 16 == 0 && H3p >= 16 && H3p % 16 == 0 && H3p <= kTAccMax && Ns >= 1 && Ns <= kTailMaxNs;
+}
+
+void tail_plan(int H3p, int *n0, int *n1) {
+    int a = H3p, b = 0;
+    if (H3p > 256) {
+        a = ((H3p / 2) + 15) / 16 * 16;
+        b = H3p - a;
+    }
+    *n0 = a;
+    *n1 = b;
+}
+
+cudaError_t launch_tail(Ctx *c, int64_t n, int64_t c0, int64_t cn, float *T, float *Y, const float *h, double dt,
+                        float *o_raw, int64_t o_stride, bool use_idx, cudaStream_t s) {
+    if (cn <= 0) return cudaSuccess;
+    TailNet &tn = c->tail;
+    TailArgs &ta = tn.args;  // the constant part (thermo, net parameters) was filled at load time
+    const LayerBf16 &l3 = c->lay[c->L - 2], &l4 = c->lay[c->L - 1];
+    ta.n = n;
+    ta.c0 = c0;
+    ta.rows = cn;
+    ta.n_active = use_idx ? c->n_active_dev : nullptr;
+    ta.idx = use_idx ? c->idx : nullptr;
+    ta.T = T;
+    ta.Y = Y;
+    ta.h = h;
+    ta.o_raw = o_raw;
+    ta.o_stride = o_stride;
+    ta.counters = c->counters;
+    for (int k = 0; k < c->Ns; ++k) {
+        ta.sA[k] = (float)(dt * (double)c->post.out_std[k]);
+        ta.sC[k] = (float)(dt * ((double)c->post.out_std[k] * (double)ta.b4[k] + (double)c->post.out_mean[k]));
+    }
+    const int64_t tiles = (cn + kTM - 1) / kTM;
+    int grid = (int)(tiles < c->sm_count ? tiles : c->sm_count);
+    grid = (grid + 1) & ~1;
+    LaunchScope ls(c, kClsTail, s);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3(kTailThreads);
+    cfg.dynamicSmemBytes = kTailSmem;
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = 2;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    (void)l4;
+    if (l4.Np <= 16) return cudaLaunchKernelEx(&cfg, k_tail<16>, l3.tmapA, tn.tmapW3a, tn.tmapW3b, tn.tmapW4, ta);
+    if (l4.Np <= 32) return cudaLaunchKernelEx(&cfg, k_tail<32>, l3.tmapA, tn.tmapW3a, tn.tmapW3b, tn.tmapW4, ta);
+    return cudaLaunchKernelEx(&cfg, k_tail<48>, l3.tmapA, tn.tmapW3a, tn.tmapW3b, tn.tmapW4, ta);
+}
+
+}  // namespace gpuann

@@ -370,7 +370,7 @@ int gpuann_load_net(gpuann_ctx *c, int n_species, int n_layers, const int *sizes
         if (!encode_tmap_bf16(&tn.tmapW3a, l3.W, (uint64_t)l3.Kp, (uint64_t)l3.Np, (uint64_t)l3.Kp * 2, (uint32_t)(ta.n0 / 2), &terr) ||
             !encode_tmap_bf16(&tn.tmapW3b, l3.W, (uint64_t)l3.Kp, (uint64_t)l3.Np, (uint64_t)l3.Kp * 2,
                               (uint32_t)(ta.n1 > 0 ? ta.n1 / 2 : 8), &terr) ||
-            !encode_tmap_bf16(&tn.tmapW4, l4.W, (uint64_t)l4.Kp, (uint64_t)l4.Np, (uint64_t)l4.Kp * 2, (uint32_t)l4.Np, &terr))
+            !encode_tmap_bf16(&tn.tmapW4, l4.W, (uint64_t)l4.Kp, (uint64_t)l4.Np, (uint64_t)l4.Kp * 2, (uint32_t)(l4.Np / 2), &terr))
             return fail(c, GPUANN_ERR_CUDA, "gpuann_load_net: " + terr);
         tn.on = true;
     }
@@ -420,6 +420,7 @@ int gpuann_load_thermo(gpuann_ctx *c, int n_species, const double *nasa_lo, cons
     {
         TailArgs &ta = c->tail.args;  // the tail kernel takes the table by value (first kTailMaxNs species)
         ta.two_ranges = h->two_ranges;
+        std::memset(&ta.th, 0, sizeof(ta.th));  // species beyond Ns of the kernel's padded range: all-zero constants
         for (int k = 0; k < kTailMaxNs && k < n_species; ++k) {
             std::memcpy(ta.th.cp[k], h->cp[k], sizeof(ta.th.cp[k]));
             std::memcpy(ta.th.hh[k], h->hh[k], sizeof(ta.th.hh[k]));

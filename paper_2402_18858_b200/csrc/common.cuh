@@ -111,7 +111,7 @@ struct TailArgs {
 };
 struct TailNet {
     bool on = false;
-    CUtensorMap tmapW3a{}, tmapW3b{}, tmapW4{};  // W3 half boxes {64, n0/2}, {64, n1/2}; W4 box {64, Np}
+    CUtensorMap tmapW3a{}, tmapW3b{}, tmapW4{};  // per-CTA boxes: W3 {64, n0/2}, {64, n1/2}; W4 {64, Np/2}
     TailArgs args{};
 };
 

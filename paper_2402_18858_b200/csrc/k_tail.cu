@@ -7,17 +7,25 @@
 // N = 32 layer-4 GEMM at 7 % of the tensor pipe behind an 80 %-of-HBM stream; here h3 goes TMEM -> registers -> a
 // 16 KB shared-memory chunk -> the layer-4 MMA, and the update runs on four warps in the shadow of the next tile's MMAs.
 //
-// Roles (512 threads, one CTA per SM in clusters of 2, 128-cell tiles walked with stride gridDim.x):
-//   warp 0       TMA: A = h2 tile k-block [128 x 64] (own) + B = W3 k-block [H3p x 64]: each CTA of the pair loads HALF
-//                of B and multicasts it to both (ring of 2); W4 [Np x K4] once, resident
-//   warp 1       layer-3 tcgen05.mma issuer + TMEM owner: acc[0..H3p) += A x B (two MMAs per k-step when H3p > 256)
-//   warp 2       layer-4 tcgen05.mma issuer: o[ob] += h3 chunk (smem) x W4 chunk (smem), two o accumulators
+// Roles (512 threads, one CTA per SM; CTA PAIRS: clusters of 2 whose even CTA, the leader, issues every tcgen05.mma with
+// cta_group::2 -- M = 256 = the 128-cell tiles of both CTAs, B read half from each CTA's shared memory, so a CTA stages
+// and reads only HALF of every W3 / W4 tile: five ring stages instead of two, half the shared-memory operand traffic):
+//   warp 0       TMA (both CTAs): A = own h2 tile k-block [128 x 64], B = own half of the W3 rows of the current column
+//                half (ring of 5), completion counted on the LEADER's full barrier; own half of W4 once, resident
+//   warp 1       (leader) layer-3 issuer + TMEM owner.  The 400 accumulator columns are two HALVES (192 + 208) with
+//                their own K loops (h2 is streamed twice, the second time from L2): while half 1 accumulates, half 0 is
+//                drained, and the next tile's half 0 starts as soon as this tile's half 1 is issued -- TMEM cannot hold
+//                two 400-column accumulators, so this is how the drain gets out of the tensor pipe's way
+//   warp 2       (leader) layer-4 issuer: o[ob] += h3 chunk (smem) x W4 chunk (smem), two o accumulators
 //   warps 4-11   drain: tcgen05.ld 32 columns of acc -> + b3 -> 2 GELU -> BF16 -> swizzled 64-column h3 chunk (ring of 2)
 //   warps 12-15  update, one thread per cell: state loads (gathered through idx under compaction) issued BEFORE waiting
 //                for o; species update in FP32 (Y^lambda by lg2/ex2, integer power 1/lambda), sum of Y* and the NASA-7
 //                MIXTURE coefficients sum_k Y_k c_kj accumulated in FP64 while the species stream by, then Newton on the
 //                two mixture polynomials in FP64: 11 FMAs per iteration instead of 11 Ns (one-range tables; a two-range
 //                table re-selects per species and iteration).  DESIGN.md "Precision of the scalar math".
+// Barriers the leader's issuers wait on live in the leader and collect arrivals (cluster-scope release) or TMA bytes
+// from BOTH CTAs; barriers that release something to a CTA's own warps are signalled in both CTAs by one multicast
+// tcgen05.commit.
 #include "common.cuh"
 #include "ptx.cuh"
 
@@ -25,17 +33,17 @@ namespace gpuann {
 
 constexpr int kTM = 128;            // cells per tile
 constexpr int kTK = 64;             // K elements per smem row (128 B)
-constexpr int kTStages = 2;
+constexpr int kTStages = 5;
 constexpr int kTAccMax = 416;       // TMEM columns of the layer-3 accumulator
 constexpr int kTOCol = 416;         // two o accumulators of kTOStride columns follow
 constexpr int kTOStride = 48;
 constexpr int kTMaxChunks = (kTAccMax + 63) / 64;  // 7
 constexpr int kTailThreads = 512;
 constexpr uint32_t kTABytes = kTM * 128;            // 16,384
-constexpr uint32_t kTBBytes = kTAccMax * 128;       // 53,248
+constexpr uint32_t kTBBytes = 128 * 128;            // this CTA's half of a column half: <= 128 rows of 128 B
 constexpr uint32_t kTStageBytes = kTABytes + kTBBytes;
 constexpr uint32_t kTH3Bytes = kTM * 128;
-constexpr uint32_t kTW4Bytes = kTMaxChunks * kTailMaxNs * 128;  // 43,008
+constexpr uint32_t kTW4Bytes = kTMaxChunks * (kTailMaxNs / 2) * 128;  // this CTA's half of the W4 rows: 21,504
 constexpr uint32_t kTOffH3 = kTStages * kTStageBytes;
 constexpr uint32_t kTOffW4 = kTOffH3 + 2 * kTH3Bytes;
 constexpr uint32_t kTOffBias = kTOffW4 + kTW4Bytes;
@@ -43,8 +51,8 @@ constexpr uint32_t kTOffBar = kTOffBias + 2048;
 constexpr size_t kTailSmem = 1024 + kTOffBar + 256;
 
 enum {
-    tFull = 0, tEmpty = tFull + kTStages, tW4Full = tEmpty + kTStages, tAccFull, tAccEmpty, tH3Full, tH3Empty = tH3Full + 2,
-    tOFull = tH3Empty + 2, tOEmpty = tOFull + 2, tCount = tOEmpty + 2
+    tFull = 0, tEmpty = tFull + kTStages, tW4Full = tEmpty + kTStages, tAccFull, tAccEmpty = tAccFull + 2,
+    tH3Full = tAccEmpty + 2, tH3Empty = tH3Full + 2, tOFull = tH3Empty + 2, tOEmpty = tOFull + 2, tCount = tOEmpty + 2
 };
 
 struct TRing {
@@ -94,7 +102,8 @@ __device__ __forceinline__ float update_species_f32(float yc, float dy, const Ta
     return (pos ? yc : 1.f) * pw;
 }
 
-template <int NSP>
+// NSP: species padded to 8.  FAST: lambda > 0 with 1/lambda = 10 and a one-range thermo table.
+template <int NSP, bool FAST>
 __global__ void __launch_bounds__(kTailThreads, 1)
 k_tail(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ CUtensorMap tmapW3a,
        const __grid_constant__ CUtensorMap tmapW3b, const __grid_constant__ CUtensorMap tmapW4,
@@ -120,16 +129,18 @@ k_tail(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ CUtens
     const int nkb = (ta.K3p + kTK - 1) / kTK;
     const int nch = (ta.H3p + 63) / 64;
 
+    const int n_half = ta.n1 > 0 ? 2 : 1;
+    const int ch0 = ta.n1 > 0 ? ta.n0 / 64 : nch;  // chunks of column half 0 (n0 is a multiple of 64 when there are two)
     if (threadIdx.x == 0) {
-        for (int i = 0; i < kTStages; ++i) { ptx::mbar_init(&bars[tFull + i], 1); ptx::mbar_init(&bars[tEmpty + i], 2); }
+        for (int i = 0; i < kTStages; ++i) { ptx::mbar_init(&bars[tFull + i], 1); ptx::mbar_init(&bars[tEmpty + i], 1); }
         ptx::mbar_init(&bars[tW4Full], 1);
-        ptx::mbar_init(&bars[tAccFull], 1);
-        ptx::mbar_init(&bars[tAccEmpty], 8);
         for (int i = 0; i < 2; ++i) {
-            ptx::mbar_init(&bars[tH3Full + i], 8);
+            ptx::mbar_init(&bars[tAccFull + i], 1);
+            ptx::mbar_init(&bars[tAccEmpty + i], 16);  // the 8 drain warps of BOTH CTAs
+            ptx::mbar_init(&bars[tH3Full + i], 16);
             ptx::mbar_init(&bars[tH3Empty + i], 1);
             ptx::mbar_init(&bars[tOFull + i], 1);
-            ptx::mbar_init(&bars[tOEmpty + i], 4);
+            ptx::mbar_init(&bars[tOEmpty + i], 8);     // the 4 update warps of both CTAs
         }
         ptx::fence_mbar_init();
     }
@@ -140,8 +151,8 @@ k_tail(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ CUtens
         ptx::prefetch_tensormap(&tmapW4);
     }
     if (warp == 1) {
-        ptx::tmem_alloc(tmem_slot, 512);
-        ptx::tmem_relinquish();
+        ptx::tmem_alloc_cg2(tmem_slot, 512);
+        ptx::tmem_relinquish_cg2();
     }
     for (int i = threadIdx.x; i < ta.H3p && i < kTAccMax; i += kTailThreads) sBias[i] = ta.bias3[i];
     ptx::tc_fence_before_sync();
@@ -150,101 +161,110 @@ k_tail(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ CUtens
     ptx::tc_fence_after_sync();
     const uint32_t tmem_base = *tmem_slot;
     const uint64_t desc0 = ptx::umma_desc_sw128_kmajor(sbase);
+    const uint32_t bars_leader = ptx::mapa_u32(ptx::smem_u32(bars), 0);  // the leader's barrier array, cluster address
+    const bool leader = crank == 0;
+
+    // register budget per warpgroup (512 threads x 128 at launch): the update warps hold a cell's whole state in registers
+    if (warp < 4) ptx::setmaxnreg_dec<104>();
+    else if (warp < 12) ptx::setmaxnreg_dec<104>();
+    else ptx::setmaxnreg_inc<200>();
 
     if (warp == 0) {
-        // ================================================================ TMA
+        // ================================================================ TMA (both CTAs)
         if (lane == 0) {
-            ptx::mbar_arrive_expect_tx(&bars[tW4Full], (uint32_t)(nch * ta.Np * 128));
+            const uint32_t sbase_cl = ptx::mapa_u32(sbase, crank);  // own shared memory in the cluster window
+            const int hp = ta.Np / 2;
+            if (leader) ptx::mbar_arrive_expect_tx(&bars[tW4Full], (uint32_t)(2 * nch * hp * 128));
             for (int c = 0; c < nch; ++c)
-                ptx::tma_load_2d(&tmapW4, &bars[tW4Full], smem + kTOffW4 + (size_t)c * ta.Np * 128, c * kTK, 0);
-            const uint32_t stage_bytes = kTABytes + (uint32_t)(ta.n0 + ta.n1) * 128u;
-            const int h0 = ta.n0 / 2, h1 = ta.n1 / 2;
+                ptx::tma_load_2d_cg2(&tmapW4, bars_leader + 8u * tW4Full, sbase_cl + kTOffW4 + (uint32_t)(c * hp * 128), c * kTK,
+                                     (int)crank * hp);
             TRing st;
             for (int it = 0; it < my_tiles; ++it) {
                 const int tile = (int)blockIdx.x + it * (int)gridDim.x;
-                for (int kb = 0; kb < nkb; ++kb) {
-                    ptx::mbar_wait(&bars[tEmpty + st.st], st.ph ^ 1u);
-                    ptx::mbar_arrive_expect_tx(&bars[tFull + st.st], stage_bytes);
-                    unsigned char *sA = smem + (size_t)st.st * kTStageBytes;
-                    unsigned char *sB = sA + kTABytes;
-                    ptx::tma_load_2d(&tmapA, &bars[tFull + st.st], sA, kb * kTK, tile * kTM);
-                    ptx::tma_load_2d_multicast(&tmapW3a, &bars[tFull + st.st], sB + (size_t)crank * h0 * 128, kb * kTK,
-                                               (int)crank * h0, 3);
-                    if (ta.n1 > 0)
-                        ptx::tma_load_2d_multicast(&tmapW3b, &bars[tFull + st.st],
-                                                   sB + (size_t)ta.n0 * 128 + (size_t)crank * h1 * 128, kb * kTK,
-                                                   ta.n0 + (int)crank * h1, 3);
-                    st.next(kTStages);
+                for (int hf = 0; hf < n_half; ++hf) {
+                    const int nh = (hf ? ta.n1 : ta.n0) / 2;  // rows of this CTA's part of the column half
+                    const int row0 = (hf ? ta.n0 : 0) + (int)crank * nh;
+                    for (int kb = 0; kb < nkb; ++kb) {
+                        ptx::mbar_wait(&bars[tEmpty + st.st], st.ph ^ 1u);
+                        if (leader) ptx::mbar_arrive_expect_tx(&bars[tFull + st.st], 2u * (kTABytes + (uint32_t)nh * 128u));
+                        const uint32_t full = bars_leader + 8u * (tFull + st.st);
+                        const uint32_t sA = sbase_cl + st.st * kTStageBytes;
+                        ptx::tma_load_2d_cg2(&tmapA, full, sA, kb * kTK, tile * kTM);
+                        ptx::tma_load_2d_cg2(hf ? &tmapW3b : &tmapW3a, full, sA + kTABytes, kb * kTK, row0);
+                        st.next(kTStages);
+                    }
                 }
             }
         }
     } else if (warp == 1) {
-        // ================================================================ layer-3 MMA issuer (whole warp, uniform)
-        const uint32_t idesc0 = ptx::umma_idesc_bf16_f32(kTM, (uint32_t)ta.n0);
-        const uint32_t idesc1 = ptx::umma_idesc_bf16_f32(kTM, (uint32_t)(ta.n1 > 0 ? ta.n1 : 16));
-        const uint64_t b1_off = (uint64_t)(((uint32_t)ta.n0 * 128u) >> 4);
-        TRing st;
-        uint32_t acc_ph = 0;
-        for (int it = 0; it < my_tiles; ++it) {
-            ptx::mbar_wait(&bars[tAccEmpty], acc_ph ^ 1u);
-            ptx::tc_fence_after_sync();
-            for (int kb = 0; kb < nkb; ++kb) {
-                ptx::mbar_wait(&bars[tFull + st.st], st.ph);
-                ptx::tc_fence_after_sync();
-                const uint64_t da = desc0 + (uint64_t)((st.st * kTStageBytes) >> 4);
-                const uint64_t db = da + (uint64_t)(kTABytes >> 4);
-                const int ksteps = min(kTK / 16, (ta.K3p - kb * kTK) / 16);
-                if (ptx::elect_one()) {
-                    if (ksteps == kTK / 16) {
+        // ================================================================ layer-3 MMA issuer (leader; whole warp, uniform)
+        if (leader) {
+            const uint32_t idesc_h[2] = {ptx::umma_idesc_bf16_f32(2 * kTM, (uint32_t)ta.n0),
+                                         ptx::umma_idesc_bf16_f32(2 * kTM, (uint32_t)(ta.n1 > 0 ? ta.n1 : 16))};
+            TRing st;
+            uint32_t acc_ph = 0;
+            for (int it = 0; it < my_tiles; ++it) {
+                for (int hf = 0; hf < n_half; ++hf) {
+                    ptx::mbar_wait_cluster(&bars[tAccEmpty + hf], acc_ph ^ 1u);
+                    ptx::tc_fence_after_sync();
+                    const uint32_t d_tmem = tmem_base + (uint32_t)(hf ? ta.n0 : 0);
+                    const uint32_t idesc = idesc_h[hf];
+                    for (int kb = 0; kb < nkb; ++kb) {
+                        ptx::mbar_wait_cluster(&bars[tFull + st.st], st.ph);
+                        ptx::tc_fence_after_sync();
+                        const uint64_t da = desc0 + (uint64_t)((st.st * kTStageBytes) >> 4);
+                        const uint64_t db = da + (uint64_t)(kTABytes >> 4);
+                        const int ksteps = min(kTK / 16, (ta.K3p - kb * kTK) / 16);
+                        if (ptx::elect_one()) {
+                            if (ksteps == kTK / 16) {
 #pragma unroll
-                        for (int k = 0; k < kTK / 16; ++k) {
-                            ptx::umma_bf16_ss(tmem_base, da + 2 * k, db + 2 * k, idesc0, (kb | k) ? 1u : 0u);
-                            if (ta.n1 > 0)
-                                ptx::umma_bf16_ss(tmem_base + (uint32_t)ta.n0, da + 2 * k, db + b1_off + 2 * k, idesc1, (kb | k) ? 1u : 0u);
+                                for (int k = 0; k < kTK / 16; ++k)
+                                    ptx::umma_bf16_ss_cg2(d_tmem, da + 2 * k, db + 2 * k, idesc, (kb | k) ? 1u : 0u);
+                            } else {
+                                for (int k = 0; k < ksteps; ++k)
+                                    ptx::umma_bf16_ss_cg2(d_tmem, da + 2 * k, db + 2 * k, idesc, (kb | k) ? 1u : 0u);
+                            }
+                            ptx::umma_commit_cg2(&bars[tEmpty + st.st], 3);
+                            if (kb == nkb - 1) ptx::umma_commit_cg2(&bars[tAccFull + hf], 3);
                         }
-                    } else {
-                        for (int k = 0; k < ksteps; ++k) {
-                            ptx::umma_bf16_ss(tmem_base, da + 2 * k, db + 2 * k, idesc0, (kb | k) ? 1u : 0u);
-                            if (ta.n1 > 0)
-                                ptx::umma_bf16_ss(tmem_base + (uint32_t)ta.n0, da + 2 * k, db + b1_off + 2 * k, idesc1, (kb | k) ? 1u : 0u);
-                        }
+                        __syncwarp();
+                        st.next(kTStages);
                     }
-                    ptx::umma_commit_multicast(&bars[tEmpty + st.st], 3);
-                    if (kb == nkb - 1) ptx::umma_commit(&bars[tAccFull]);
                 }
-                __syncwarp();
-                st.next(kTStages);
+                acc_ph ^= 1u;
             }
-            acc_ph ^= 1u;
         }
     } else if (warp == 2) {
-        // ================================================================ layer-4 MMA issuer (whole warp, uniform)
-        const uint32_t idesc4 = ptx::umma_idesc_bf16_f32(kTM, (uint32_t)ta.Np);
-        ptx::mbar_wait(&bars[tW4Full], 0);
-        uint32_t seq = 0;
-        for (int it = 0; it < my_tiles; ++it) {
-            const uint32_t ob = (uint32_t)it & 1u, oph = ((uint32_t)it >> 1) & 1u;
-            ptx::mbar_wait(&bars[tOEmpty + ob], oph ^ 1u);
-            ptx::tc_fence_after_sync();
-            const uint32_t d_tmem = tmem_base + kTOCol + ob * kTOStride;
-            for (int c = 0; c < nch; ++c, ++seq) {
-                const uint32_t buf = seq & 1u, ph = (seq >> 1) & 1u;
-                ptx::mbar_wait(&bars[tH3Full + buf], ph);
+        // ================================================================ layer-4 MMA issuer (leader; whole warp, uniform)
+        if (leader) {
+            const uint32_t idesc4 = ptx::umma_idesc_bf16_f32(2 * kTM, (uint32_t)ta.Np);
+            ptx::mbar_wait_cluster(&bars[tW4Full], 0);
+            const uint32_t w4_chunk = (uint32_t)(ta.Np / 2) * 128u;
+            uint32_t seq = 0;
+            for (int it = 0; it < my_tiles; ++it) {
+                const uint32_t ob = (uint32_t)it & 1u, oph = ((uint32_t)it >> 1) & 1u;
+                ptx::mbar_wait_cluster(&bars[tOEmpty + ob], oph ^ 1u);
                 ptx::tc_fence_after_sync();
-                const uint64_t da = desc0 + (uint64_t)((kTOffH3 + buf * kTH3Bytes) >> 4);
-                const uint64_t db = desc0 + (uint64_t)((kTOffW4 + (uint32_t)c * (uint32_t)ta.Np * 128u) >> 4);
-                const int ksteps = min(4, (ta.H3p - c * 64) / 16);
-                if (ptx::elect_one()) {
-                    for (int k = 0; k < ksteps; ++k)
-                        ptx::umma_bf16_ss(d_tmem, da + 2 * k, db + 2 * k, idesc4, (c | k) ? 1u : 0u);
-                    ptx::umma_commit(&bars[tH3Empty + buf]);
-                    if (c == nch - 1) ptx::umma_commit(&bars[tOFull + ob]);
+                const uint32_t d_tmem = tmem_base + kTOCol + ob * kTOStride;
+                for (int c = 0; c < nch; ++c, ++seq) {
+                    const uint32_t buf = seq & 1u, ph = (seq >> 1) & 1u;
+                    ptx::mbar_wait_cluster(&bars[tH3Full + buf], ph);
+                    ptx::tc_fence_after_sync();
+                    const uint64_t da = desc0 + (uint64_t)((kTOffH3 + buf * kTH3Bytes) >> 4);
+                    const uint64_t db = desc0 + (uint64_t)((kTOffW4 + (uint32_t)c * w4_chunk) >> 4);
+                    const int ksteps = min(4, (ta.H3p - c * 64) / 16);
+                    if (ptx::elect_one()) {
+                        for (int k = 0; k < ksteps; ++k)
+                            ptx::umma_bf16_ss_cg2(d_tmem, da + 2 * k, db + 2 * k, idesc4, (c | k) ? 1u : 0u);
+                        ptx::umma_commit_cg2(&bars[tH3Empty + buf], 3);
+                        if (c == nch - 1) ptx::umma_commit_cg2(&bars[tOFull + ob], 3);
+                    }
+                    __syncwarp();
                 }
-                __syncwarp();
             }
         }
     } else if (warp >= 4 && warp < 12) {
-        // ================================================================ drain: acc -> h3 chunks (warps 4..11)
+        // ================================================================ drain: acc -> h3 chunks (warps 4..11, both CTAs)
         const int q = warp & 3;           // TMEM lane quarter
         const int hsel = (warp - 4) >> 2; // which 32-column half of every 64-column chunk
         const int r = q * 32 + lane;
@@ -253,11 +273,12 @@ k_tail(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ CUtens
         const uint32_t row_off = (uint32_t)r * 128u;
         uint32_t acc_ph = 0, seq = 0;
         for (int it = 0; it < my_tiles; ++it) {
-            ptx::mbar_wait(&bars[tAccFull], acc_ph);
-            ptx::tc_fence_after_sync();
-            acc_ph ^= 1u;
 #pragma unroll 1
             for (int c = 0; c < nch; ++c, ++seq) {
+                if (c == 0 || c == ch0) {  // first chunk of a column half: wait for its accumulator
+                    ptx::mbar_wait(&bars[tAccFull + (c == 0 ? 0 : 1)], acc_ph);
+                    ptx::tc_fence_after_sync();
+                }
                 const int cc = c * 64 + hsel * 32;
                 const int w = ta.H3p - cc;  // >= 32: full piece; 16: half piece; <= 0: none (widths are multiples of 16)
                 uint32_t v[32];
@@ -274,10 +295,10 @@ k_tail(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ CUtens
                     for (int j = 0; j < 32; ++j) v[j] = 0u;
                 }
                 ptx::tmem_ld_wait();
-                if (c == nch - 1) {  // last accumulator read of this warp in this tile
+                if (c == ch0 - 1 || c == nch - 1) {  // last read of a column half by this warp: hand it back to the issuer
                     ptx::tc_fence_before_sync();
                     __syncwarp();
-                    if (lane == 0) ptx::mbar_arrive(&bars[tAccEmpty]);
+                    if (lane == 0) ptx::mbar_arrive_cluster(bars_leader + 8u * (tAccEmpty + ((c == nch - 1 && n_half == 2) ? 1 : 0)));
                 }
                 uint32_t o[16];
                 if (w > 0) {
@@ -301,15 +322,19 @@ k_tail(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ CUtens
                     ptx::fence_proxy_async_smem();
                 }
                 __syncwarp();
-                if (lane == 0) ptx::mbar_arrive(&bars[tH3Full + buf]);
+                if (lane == 0) ptx::mbar_arrive_cluster(bars_leader + 8u * (tH3Full + buf));
             }
+            acc_ph ^= 1u;
         }
     } else if (warp >= 12) {
         // ================================================================ update S4-S8 (warps 12..15), one thread per cell
+        // Species k >= Ns of the padded range carry Y = 0, o = 0 and all-zero constants: they produce Y* = 0 and drop out
+        // of every sum, so the arithmetic below has no per-species guards (only the loads and stores are predicated).
         const int q = warp & 3;
         const int r = q * 32 + lane;
         const uint32_t lane_addr = tmem_base + ((uint32_t)(q * 32) << 16) + kTOCol;
         const int Ns = ta.Ns;
+        const bool fwd_only = ta.o_raw != nullptr;
         unsigned nconv_total = 0, ndeg_total = 0;
         for (int it = 0; it < my_tiles; ++it) {
             const int tile = (int)blockIdx.x + it * (int)gridDim.x;
@@ -319,7 +344,6 @@ k_tail(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ CUtens
             if (ta.idx) g = valid ? (int64_t)ta.idx[g] : 0;
             if (!valid) g = 0;
             const uint32_t ob = (uint32_t)it & 1u, oph = ((uint32_t)it >> 1) & 1u;
-            const bool fwd_only = ta.o_raw != nullptr;
             // state loads first: their latency hides behind the wait for o
             float Yv[NSP];
             float Tin = 300.f, hin = 0.f;
@@ -333,70 +357,76 @@ k_tail(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ CUtens
             }
             ptx::mbar_wait(&bars[tOFull + ob], oph);
             ptx::tc_fence_after_sync();
+            // S4 + S5 (R3, R7) in FP32; sum of Y* and the mixture coefficients sum_k Y*_k c_kj in FP64; o is read from TMEM
+            // eight species at a time
             double S = 0.0;
             double Ch[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0}, Cc[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
 #pragma unroll
-            for (int pc = 0; pc < NSP / 16; ++pc) {
-                uint32_t ov[16];
-                ptx::tmem_ld16(lane_addr + ob * kTOStride + (uint32_t)(16 * pc), ov);
+            for (int pc = 0; pc < NSP / 8; ++pc) {
+                uint32_t t8[8];
+                ptx::tmem_ld8(lane_addr + ob * kTOStride + (uint32_t)(8 * pc), t8);
                 ptx::tmem_ld_wait();
-                if (pc == NSP / 16 - 1) {  // o is in registers: hand the accumulator back to the layer-4 issuer
+                if (pc == NSP / 8 - 1) {  // o is in registers: hand the accumulator back to the layer-4 issuer
                     ptx::tc_fence_before_sync();
                     __syncwarp();
-                    if (lane == 0) ptx::mbar_arrive(&bars[tOEmpty + ob]);
+                    if (lane == 0) ptx::mbar_arrive_cluster(bars_leader + 8u * (tOEmpty + ob));
                 }
 #pragma unroll
-                for (int j = 0; j < 16; ++j) {
-                    const int k = 16 * pc + j;
-                    if (k < Ns) {
-                        const float o = __uint_as_float(ov[j]);
-                        if (fwd_only) {
-                            if (valid) ta.o_raw[(int64_t)k * ta.o_stride + i] = o + ta.b4[k];
-                        } else {
-                            const float ys = update_species_f32(fmaxf(Yv[k], 0.f), fmaf(o, ta.sA[k], ta.sC[k]), ta);
-                            Yv[k] = ys;
-                            const double yd = (double)ys;
-                            S += yd;
-                            if (!ta.two_ranges) {
+                for (int j = 0; j < 8; ++j) {
+                    const int k = 8 * pc + j;
+                    const float o = __uint_as_float(t8[j]);
+                    if (fwd_only) {
+                        if (valid && k < Ns) ta.o_raw[(int64_t)k * ta.o_stride + i] = o + ta.b4[k];
+                        continue;
+                    }
+                    const float yc = fmaxf(Yv[k], 0.f);
+                    const float dy = fmaf(o, ta.sA[k], ta.sC[k]);
+                    float ys;
+                    if (FAST) {
+                        // lambda = 1/10: Y* = Yc (max(1 + lambda dy / u, 0))^10, u = Yc^lambda = ex2(lambda lg2 Yc); Yc = 0 (or
+                        // so small that u flushes to 0): Y* = max(lambda dy, 0)^10.  lg2(0) = -inf, ex2(-inf) = 0: no guard
+                        const float u = ptx::ex2_approx(ta.lambda * ptx::lg2_approx(yc));
+                        const float ldy = ta.lambda * dy;
+                        const bool pos = u > 0.f;
+                        const float base = fmaxf(pos ? fmaf(ldy, ptx::rcp_approx(u), 1.f) : ldy, 0.f);
+                        const float b2 = base * base, b4 = b2 * b2;
+                        ys = (pos ? yc : 1.f) * (b4 * b4 * b2);
+                    } else {
+                        ys = update_species_f32(yc, dy, ta);
+                    }
+                    Yv[k] = ys;
+                    const double yd = (double)ys;
+                    S += yd;
+                    if (FAST || !ta.two_ranges) {
 #pragma unroll
-                                for (int m = 0; m < 6; ++m) Ch[m] = fma(yd, ta.th.hh[k][0][m], Ch[m]);
+                        for (int m = 0; m < 6; ++m) Ch[m] = fma(yd, ta.th.hh[k][0][m], Ch[m]);
 #pragma unroll
-                                for (int m = 0; m < 5; ++m) Cc[m] = fma(yd, ta.th.cp[k][0][m], Cc[m]);
-                            }
-                        }
+                        for (int m = 0; m < 5; ++m) Cc[m] = fma(yd, ta.th.cp[k][0][m], Cc[m]);
                     }
                 }
             }
             if (fwd_only) continue;
             // S6 (R8): divide by the sum; a vanishing sum falls back to max(Y,0)/sum (rare: the inputs are re-read)
             const bool degenerate = !(S > 0.0);
-            double rS;
-            if (!degenerate) {
-                rS = 1.0 / S;
-            } else {
-                double Sc = 0.0;
-#pragma unroll
-                for (int k = 0; k < NSP; ++k) {
-                    Yv[k] = (valid && k < Ns) ? fmaxf(ta.Y[(int64_t)k * ta.n + g], 0.f) : 0.f;
-                    Sc += (double)Yv[k];
-                }
-                rS = 1.0 / Sc;
+            if (degenerate) {
+                S = 0.0;
 #pragma unroll
                 for (int m = 0; m < 6; ++m) Ch[m] = 0.0;
 #pragma unroll
                 for (int m = 0; m < 5; ++m) Cc[m] = 0.0;
-                if (!ta.two_ranges) {
+#pragma unroll 1
+                for (int k = 0; k < Ns; ++k) S += (double)fmaxf(valid ? ta.Y[(int64_t)k * ta.n + g] : 0.f, 0.f);
 #pragma unroll
-                    for (int k = 0; k < NSP; ++k)
-                        if (k < Ns) {
-                            const double yd = (double)Yv[k];
+                for (int k = 0; k < NSP; ++k) {
+                    Yv[k] = (valid && k < Ns) ? fmaxf(ta.Y[(int64_t)k * ta.n + g], 0.f) : 0.f;
+                    const double yd = (double)Yv[k];
 #pragma unroll
-                            for (int m = 0; m < 6; ++m) Ch[m] = fma(yd, ta.th.hh[k][0][m], Ch[m]);
+                    for (int m = 0; m < 6; ++m) Ch[m] = fma(yd, ta.th.hh[k][0][m], Ch[m]);
 #pragma unroll
-                            for (int m = 0; m < 5; ++m) Cc[m] = fma(yd, ta.th.cp[k][0][m], Cc[m]);
-                        }
+                    for (int m = 0; m < 5; ++m) Cc[m] = fma(yd, ta.th.cp[k][0][m], Cc[m]);
                 }
             }
+            const double rS = 1.0 / S;
 #pragma unroll
             for (int m = 0; m < 6; ++m) Ch[m] *= rS;
 #pragma unroll
@@ -407,20 +437,19 @@ k_tail(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ CUtens
             const double hc = (double)hin;
             for (int itn = 0; itn < ta.newton_max_iter; ++itn) {
                 double f, c;
-                if (!ta.two_ranges) {
+                if (FAST || !ta.two_ranges) {
                     f = horner6(Ch, Tn) - hc;
                     c = horner5(Cc, Tn);
                 } else {
                     f = 0.0;
                     c = 0.0;
 #pragma unroll
-                    for (int k = 0; k < NSP; ++k)
-                        if (k < Ns) {
-                            const int rg = !(Tn < ta.th.T_mid[k]) ? 1 : 0;
-                            const double yd = (double)Yv[k] * rS;
-                            f = fma(yd, horner6(ta.th.hh[k][rg], Tn), f);
-                            c = fma(yd, horner5(ta.th.cp[k][rg], Tn), c);
-                        }
+                    for (int k = 0; k < NSP; ++k) {
+                        const int rg = (k < Ns && !(Tn < ta.th.T_mid[k])) ? 1 : 0;
+                        const double yd = (double)Yv[k] * rS;
+                        f = fma(yd, horner6(ta.th.hh[k][rg], Tn), f);
+                        c = fma(yd, horner5(ta.th.cp[k][rg], Tn), c);
+                    }
                     f -= hc;
                 }
                 if (!(c > 0.0)) break;  // R10: stop, not converged
@@ -452,30 +481,46 @@ k_tail(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ CUtens
 
     ptx::tc_fence_before_sync();
     __syncthreads();
-    ptx::cluster_sync_all();  // no CTA leaves while its peer may still multicast into it or signal its barriers
+    ptx::cluster_sync_all();  // no CTA leaves while its peer may still signal its barriers or the pair's MMAs run
     if (warp == 1) {
         ptx::tc_fence_after_sync();
-        ptx::tmem_dealloc(tmem_base, 512);
+        ptx::tmem_dealloc_cg2(tmem_base, 512);
     }
 }
 
 // ---------------------------------------------------------------- host side
+typedef void (*TailKernel)(const CUtensorMap, const CUtensorMap, const CUtensorMap, const CUtensorMap, const TailArgs);
+
+static TailKernel tail_kernel(int Ns, bool fast) {
+    switch ((Ns + 7) / 8) {
+        case 1: return fast ? k_tail<8, true> : k_tail<8, false>;
+        case 2: return fast ? k_tail<16, true> : k_tail<16, false>;
+        case 3: return fast ? k_tail<24, true> : k_tail<24, false>;
+        case 4: return fast ? k_tail<32, true> : k_tail<32, false>;
+        case 5: return fast ? k_tail<40, true> : k_tail<40, false>;
+        default: return fast ? k_tail<48, true> : k_tail<48, false>;
+    }
+}
+
 cudaError_t tail_setup(Ctx *c) {
     (void)c;
-    cudaError_t e = cudaFuncSetAttribute(k_tail<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTailSmem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_tail<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTailSmem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_tail<48>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTailSmem);
-    return e;
+    for (int ns = 8; ns <= kTailMaxNs; ns += 8)
+        for (int fast = 0; fast < 2; ++fast) {
+            cudaError_t e = cudaFuncSetAttribute(tail_kernel(ns, fast != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTailSmem);
+            if (e != cudaSuccess) return e;
+        }
+    return cudaSuccess;
 }
 
 bool tail_supported(int K3p, int H3p, int Ns) {
     return K3p >= 16 && K3p % 16 == 0 && H3p >= 16 && H3p % 16 == 0 && H3p <= kTAccMax && Ns >= 1 && Ns <= kTailMaxNs;
 }
 
+// column halves of the layer-3 accumulator: one (<= 256 columns), or two with the first on a 64-column chunk boundary
 void tail_plan(int H3p, int *n0, int *n1) {
     int a = H3p, b = 0;
     if (H3p > 256) {
-        a = ((H3p / 2) + 15) / 16 * 16;
+        a = ((H3p + 63) / 64 / 2) * 64;
         b = H3p - a;
     }
     *n0 = a;
@@ -520,9 +565,10 @@ cudaError_t launch_tail(Ctx *c, int64_t n, int64_t c0, int64_t cn, float *T, flo
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     (void)l4;
-    if (l4.Np <= 16) return cudaLaunchKernelEx(&cfg, k_tail<16>, l3.tmapA, tn.tmapW3a, tn.tmapW3b, tn.tmapW4, ta);
-    if (l4.Np <= 32) return cudaLaunchKernelEx(&cfg, k_tail<32>, l3.tmapA, tn.tmapW3a, tn.tmapW3b, tn.tmapW4, ta);
-    return cudaLaunchKernelEx(&cfg, k_tail<48>, l3.tmapA, tn.tmapW3a, tn.tmapW3b, tn.tmapW4, ta);
+    // species beyond Ns of the padded range must carry all-zero constants (the kernel's arithmetic is unguarded)
+    for (int k = c->Ns; k < kTailMaxNs; ++k) ta.sA[k] = ta.sC[k] = 0.f;
+    const bool fast = !ta.lambda_zero && ta.inv_lambda_int == 10 && !ta.two_ranges;
+    return cudaLaunchKernelEx(&cfg, tail_kernel(c->Ns, fast), l3.tmapA, tn.tmapW3a, tn.tmapW3b, tn.tmapW4, ta);
 }
 
 }  // namespace gpuann

@@ -302,7 +302,8 @@ int gpuann_load_net(gpuann_ctx *c, int n_species, int n_layers, const int *sizes
         fused_plan(c->lay[1].Np, &fn.n_pass, &fn.pass_w, &fn.n0, &fn.n1);
         // W1 padded to K = 64 with the bias in two extra columns: b1 = hi + lo, both BF16, multiplied by the
         // constant-1 features z[D], z[D+1] the kernel appends (bias error <= 2^-17 |b1|)
-        std::vector<uint16_t> w1((size_t)H1 * 64, 0);
+        const int H1p = (H1 + 63) / 64 * 64;  // rows up to the next multiple of 64 stay zero: h1 = 0 there (k_fused.cu)
+        std::vector<uint16_t> w1((size_t)H1p * 64, 0);
         for (int j = 0; j < H1; ++j) {
             for (int i = 0; i < D; ++i) w1[(size_t)j * 64 + i] = f32_to_bf16_rne(weights[0][(size_t)j * D + i]);
             const float b = biases[0][j];
@@ -317,8 +318,8 @@ int gpuann_load_net(gpuann_ctx *c, int n_species, int n_layers, const int *sizes
         CU_TRY(c, cudaMemcpy(fn.W1p, w1.data(), w1.size() * sizeof(uint16_t), cudaMemcpyHostToDevice), "cudaMemcpy(W1 padded)");
         std::string terr;
         const LayerBf16 &l2 = c->lay[1];
-        // boxes are HALF stages: each CTA of a pair loads one half and multicasts it to both (k_fused.cu)
-        if (!encode_tmap_bf16(&fn.tmapW1, fn.W1p, 64, (uint64_t)H1, 128, 32, &terr) ||
+        // boxes are a CTA's HALF of a stage: the pair's MMAs (cta_group::2) read half of B from each CTA (k_fused.cu)
+        if (!encode_tmap_bf16(&fn.tmapW1, fn.W1p, 64, (uint64_t)H1p, 128, 16, &terr) ||
             !encode_tmap_bf16(&fn.tmapW2a, l2.W, (uint64_t)l2.Kp, (uint64_t)l2.Np, (uint64_t)l2.Kp * 2, (uint32_t)(fn.n0 / 2), &terr) ||
             !encode_tmap_bf16(&fn.tmapW2b, l2.W, (uint64_t)l2.Kp, (uint64_t)l2.Np, (uint64_t)l2.Kp * 2,
                               (uint32_t)(fn.n1 > 0 ? fn.n1 / 2 : 8), &terr))
@@ -326,8 +327,8 @@ int gpuann_load_net(gpuann_ctx *c, int n_species, int n_layers, const int *sizes
         fn.on = true;
         // MACs issued: layer 1 once per pass over 16 * Kz columns, layer 2 over n_pass * pass_w columns
         const int Kz16 = ((D + 2 + 15) / 16) * 16;
-        mac += (int64_t)fn.n_pass * H1 * Kz16 - (int64_t)c->lay[0].Kp * c->lay[0].Np;
-        mac += (int64_t)H1 * ((int64_t)fn.n_pass * fn.pass_w - l2.Np);
+        mac += (int64_t)fn.n_pass * H1p * Kz16 - (int64_t)c->lay[0].Kp * c->lay[0].Np;
+        mac += (int64_t)H1p * (int64_t)fn.n_pass * fn.pass_w - (int64_t)l2.Kp * l2.Np;
     }
     // activation scratch: ping-pong buffers [chunk][maxKp]; with the fused kernel in front and the tail kernel behind
     // only ONE of them is ever used (h2), and the raw output never leaves the SM

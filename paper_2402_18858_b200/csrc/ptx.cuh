@@ -73,6 +73,24 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
     }
 }
 
+// Blocks until both phases have completed; the two polls are issued back to back so that their latencies overlap.
+__device__ __forceinline__ void mbar_wait2(uint64_t *bar_a, uint32_t parity_a, uint64_t *bar_b, uint32_t parity_b) {
+    uint32_t a, b;
+    do {
+        asm volatile(
+            "{\n\t"
+            ".reg .pred p, q;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%2], %3;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 q, [%4], %5;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t"
+            "selp.u32 %1, 1, 0, q;\n\t"
+            "}\n"
+            : "=r"(a), "=r"(b)
+            : "r"(smem_u32(bar_a)), "r"(parity_a), "r"(smem_u32(bar_b)), "r"(parity_b)
+            : "memory");
+    } while (!(a & b));
+}
+
 // generic-proxy writes to shared memory (st.shared) -> visible to the async proxy (tcgen05.mma, TMA)
 __device__ __forceinline__ void fence_proxy_async_smem() {
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -110,24 +128,18 @@ __device__ __forceinline__ uint32_t mapa_u32(uint32_t local_smem_addr, uint32_t 
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local_smem_addr), "r"(cta));
     return r;
 }
-// arrive (release at cluster scope) on an mbarrier given by its shared::cluster address (own or peer CTA)
+// arrive on an mbarrier given by its shared::cluster address (own or peer CTA).  Default semantics (release at CTA scope), as
+// CUTLASS's ClusterBarrier::arrive: what the arrivals of this library hand over is tensor memory (ordered by tcgen05.wait /
+// tcgen05.fence) or shared memory that only the async proxy reads (ordered by fence.proxy.async), never generic-proxy data
+// of the peer.  The .release.cluster / .acquire.cluster forms cost ~1000 clk per arrive behind outstanding global stores and
+// a CCTL.IVALL (L1 invalidate) per successful wait (profiles/r02_fused.md).
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
-    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+    asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
 }
-// wait with acquire at cluster scope (the phase may have been completed by arrivals from the peer CTA)
+// wait on an mbarrier of this CTA whose phase may be completed by arrivals / TMA bytes from the peer CTA
 __device__ __forceinline__ void mbar_wait_cluster(uint64_t *bar, uint32_t parity) {
-    uint32_t ok;
-    do {
-        asm volatile(
-            "{\n\t"
-            ".reg .pred p;\n\t"
-            "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\t"
-            "selp.u32 %0, 1, 0, p;\n\t"
-            "}\n"
-            : "=r"(ok)
-            : "r"(smem_u32(bar)), "r"(parity)
-            : "memory");
-    } while (!ok);
+    while (!mbar_try_wait(bar, parity)) {
+    }
 }
 // TMA tile load into THIS CTA's shared memory whose completion (complete_tx) is signalled on an mbarrier of either
 // CTA of the pair, given by its shared::cluster address (the leader's "full" barrier counts the bytes of both CTAs)
@@ -161,6 +173,19 @@ __device__ __forceinline__ void umma_bf16_ss_cg2(uint32_t tmem_d, uint64_t desc_
         "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t"
         "}\n" ::"r"(tmem_d),
         "l"(desc_a), "l"(desc_b), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+// the same with the A operand in TENSOR MEMORY (each CTA's 128 rows of A at tmem_a in its own TMEM: lane = row, one 32-bit
+// column = two consecutive K elements, 8 columns per K = 16 step) -- no shared-memory read for A
+__device__ __forceinline__ void umma_bf16_ts_cg2(uint32_t tmem_d, uint32_t tmem_a, uint64_t desc_b, uint32_t idesc,
+                                                 uint32_t accumulate) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::2.kind::f16 [%0], [%1], %2, %3, p;\n\t"
+        "}\n" ::"r"(tmem_d),
+        "r"(tmem_a), "l"(desc_b), "r"(idesc), "r"(accumulate)
         : "memory");
 }
 // arrives on the mbarrier at the same offset in every CTA of cta_mask when all MMAs issued so far by this thread are done
@@ -284,6 +309,19 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
           "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
         : "r"(taddr)
         : "memory");
+}
+
+// registers -> TMEM: 32 lanes x 32 bit, 16 consecutive columns (thread t of the warp writes lane base_lane + t)
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&v)[16]) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
+        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};" ::"r"(taddr),
+        "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]), "r"(v[9]),
+        "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15])
+        : "memory");
+}
+__device__ __forceinline__ void tmem_st_wait() {
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
 }
 
 __device__ __forceinline__ void tmem_ld_wait() {

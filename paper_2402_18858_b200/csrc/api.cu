@@ -373,6 +373,11 @@ int gpuann_load_net(gpuann_ctx *c, int n_species, int n_layers, const int *sizes
                               (uint32_t)(ta.n1 > 0 ? ta.n1 / 2 : 8), &terr) ||
             !encode_tmap_bf16(&tn.tmapW4, l4.W, (uint64_t)l4.Kp, (uint64_t)l4.Np, (uint64_t)l4.Kp * 2, (uint32_t)(l4.Np / 2), &terr))
             return fail(c, GPUANN_ERR_CUDA, "gpuann_load_net: " + terr);
+        // fused kernel directly in front: h2 travels in the blocked layout (common.cuh, FusedNet)
+        ta.a_blocked = one_buffer ? 1 : 0;
+        c->fused.h2_blocked = one_buffer;
+        if (one_buffer && !encode_tmap_bf16_linear(&tn.tmapAb, c->act[0], (uint64_t)chunk * (uint64_t)l3.Kp, &terr))
+            return fail(c, GPUANN_ERR_CUDA, "gpuann_load_net: " + terr);
         tn.on = true;
     }
     c->issued_mac_per_cell = mac;

@@ -80,6 +80,13 @@ struct FusedNet {
     CUtensorMap tmapW1{};          // box {64, 64}
     CUtensorMap tmapW2a{}, tmapW2b{};  // W2 [H2p][H1]: box {64, n0}, box {64, n1}
     int n_pass = 0, pass_w = 0, n0 = 0, n1 = 0;
+    // h2 layout in HBM when the tail kernel consumes it directly: BLOCKED in the MMA's canonical core-matrix order,
+    //     h2b[tile][kp = column / 8][row 0..127][8 columns]   (16-byte pieces; a (tile, kp) slab is 2 KB)
+    // so that (a) a drain warp's store instruction -- lane = row, one 16-byte piece -- writes 512 contiguous bytes instead
+    // of 32 pieces 1600 bytes apart (the row-major stores cost 6,400 LSU line transactions per pass and made the drain
+    // 10 k clk long; profiles/r02_fused.md), and (b) a [128 x 64] A stage of the tail kernel is ONE contiguous 16 KB
+    // piece of global memory, read by the MMA through a no-swizzle descriptor (LBO 2048, SBO 128).
+    bool h2_blocked = false;
 };
 
 // tail kernel (k_tail.cu): the last two layers + S4-S8.  TailArgs is the kernel's by-value parameter block: the
@@ -99,6 +106,7 @@ struct TailArgs {
     int64_t o_stride;
     int Ns, Np;    // species, padded to 16
     int K3p, H3p, n0, n1;
+    int a_blocked;  // 1: the input activation is in the blocked layout the fused kernel writes (see FusedNet)
     const float *bias3;
     int newton_max_iter, inv_lambda_int, lambda_zero, two_ranges;
     float lambda, inv_lambda;
@@ -112,6 +120,7 @@ struct TailArgs {
 struct TailNet {
     bool on = false;
     CUtensorMap tmapW3a{}, tmapW3b{}, tmapW4{};  // per-CTA boxes: W3 {64, n0/2}, {64, n1/2}; W4 {64, Np/2}
+    CUtensorMap tmapAb{};                        // the kernel's input in the BLOCKED layout (see h2 layout below)
     TailArgs args{};
 };
 
@@ -257,5 +266,8 @@ cudaError_t launch_tail(Ctx *c, int64_t n, int64_t c0, int64_t cn, float *T, flo
 // encodes a 2-D BF16 row-major tensor map {inner = cols, outer = rows}, box {64, box_rows}, 128-byte swizzle
 bool encode_tmap_bf16(CUtensorMap *out, const void *base, uint64_t cols, uint64_t rows, uint64_t row_pitch_bytes,
                       uint32_t box_rows, std::string *err);
+
+// 2-D map over `total_elems` contiguous BF16 viewed as rows of 256: box {256, 32} = 16 KB contiguous, no swizzle
+bool encode_tmap_bf16_linear(CUtensorMap *out, const void *base, uint64_t total_elems, std::string *err);
 
 }  // namespace gpuann

@@ -91,7 +91,8 @@ struct FusedArgs {
     int H1p, H2p;            // H1 padded to a multiple of 64 (zero rows of W1, zero-filled K columns of W2); padded H2
     int n_pass, pass_w, n0, n1;
     const float *bias2;      // [H2p]
-    __nv_bfloat16 *h2;       // [rows][H2p]
+    __nv_bfloat16 *h2;       // [rows][H2p] row-major, or blocked [tile][H2p / 8][128][8] (common.cuh, FusedNet)
+    int h2_blocked;
     PreParams pre;
 };
 
@@ -420,7 +421,19 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
                     o[2 * jj] = ptx::gelu2_pack(__uint_as_float(v[4 * jj]) + bb.x, __uint_as_float(v[4 * jj + 1]) + bb.y);
                     o[2 * jj + 1] = ptx::gelu2_pack(__uint_as_float(v[4 * jj + 2]) + bb.z, __uint_as_float(v[4 * jj + 3]) + bb.w);
                 }
-                if (row_ok) {
+                if (fa.h2_blocked) {
+                    // lane = row, one 16-byte piece per instruction: 512 contiguous bytes per warp instruction.  Rows past
+                    // the end of a real tile are stored too (the buffer holds whole tiles; they are zeros)
+                    if (tile < n_tiles) {
+                        uint4 *dst = reinterpret_cast<uint4 *>(fa.h2) + ((int64_t)tile * (fa.H2p >> 3) + ((col_base + cc) >> 3)) * kFM + r;
+                        dst[0] = make_uint4(o[0], o[1], o[2], o[3]);
+                        dst[kFM] = make_uint4(o[4], o[5], o[6], o[7]);
+                        if (full) {
+                            dst[2 * kFM] = make_uint4(o[8], o[9], o[10], o[11]);
+                            dst[3 * kFM] = make_uint4(o[12], o[13], o[14], o[15]);
+                        }
+                    }
+                } else if (row_ok) {
                     uint4 *dst = reinterpret_cast<uint4 *>(dst_row + cc);
                     dst[0] = make_uint4(o[0], o[1], o[2], o[3]);
                     dst[1] = make_uint4(o[4], o[5], o[6], o[7]);
@@ -518,6 +531,7 @@ cudaError_t launch_fused_l1l2(Ctx *c, int64_t n, int64_t c0, int64_t cn, const f
     fa.n1 = fn.n1;
     fa.bias2 = c->lay[1].bias;
     fa.h2 = c->act[0];
+    fa.h2_blocked = fn.h2_blocked ? 1 : 0;
     fa.pre = c->pre;
     const int64_t tiles = (cn + kFM - 1) / kFM;
     int grid = (int)(tiles < c->sm_count ? tiles : c->sm_count);

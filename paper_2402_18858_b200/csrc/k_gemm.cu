@@ -297,6 +297,23 @@ bool encode_tmap_bf16(CUtensorMap *out, const void *base, uint64_t cols, uint64_
     return true;
 }
 
+bool encode_tmap_bf16_linear(CUtensorMap *out, const void *base, uint64_t total_elems, std::string *err) {
+    PFN_encodeTiled fn = get_encode_fn(err);
+    if (!fn) return false;
+    cuuint64_t dims[2] = {256, total_elems / 256};
+    cuuint64_t strides[1] = {512};
+    cuuint32_t box[2] = {256, 32};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = fn(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void *>(base), dims, strides, box, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        if (err) *err = "cuTensorMapEncodeTiled (linear) failed with CUresult " + std::to_string((int)r);
+        return false;
+    }
+    return true;
+}
+
 cudaError_t gemm_setup(Ctx *c) {
     (void)c;
     return cudaFuncSetAttribute(k_layer_bf16, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kGemmSmem);

@@ -105,7 +105,8 @@ __device__ __forceinline__ float update_species_f32(float yc, float dy, const Ta
 // NSP: species padded to 8.  FAST: lambda > 0 with 1/lambda = 10 and a one-range thermo table.
 template <int NSP, bool FAST>
 __global__ void __launch_bounds__(kTailThreads, 1)
-k_tail(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ CUtensorMap tmapW3a,
+k_tail(const __grid_constant__ CUtensorMap tmapA /* row-major [rows][K3p] or blocked (common.cuh, FusedNet) */,
+       const __grid_constant__ CUtensorMap tmapW3a,
        const __grid_constant__ CUtensorMap tmapW3b, const __grid_constant__ CUtensorMap tmapW4,
        const __grid_constant__ TailArgs ta) {
     extern __shared__ unsigned char smem_raw[];
@@ -161,6 +162,7 @@ k_tail(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ CUtens
     ptx::tc_fence_after_sync();
     const uint32_t tmem_base = *tmem_slot;
     const uint64_t desc0 = ptx::umma_desc_sw128_kmajor(sbase);
+    const uint64_t descA0 = ptx::umma_desc_nosw_kmajor(sbase, 2048, 128);  // blocked A stage: [8 kp][128 rows][16 B]
     const uint32_t bars_leader = ptx::mapa_u32(ptx::smem_u32(bars), 0);  // the leader's barrier array, cluster address
     const bool leader = crank == 0;
 
@@ -189,7 +191,10 @@ k_tail(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ CUtens
                         if (leader) ptx::mbar_arrive_expect_tx(&bars[tFull + st.st], 2u * (kTABytes + (uint32_t)nh * 128u));
                         const uint32_t full = bars_leader + 8u * (tFull + st.st);
                         const uint32_t sA = sbase_cl + st.st * kTStageBytes;
-                        ptx::tma_load_2d_cg2(&tmapA, full, sA, kb * kTK, tile * kTM);
+                        if (ta.a_blocked)  // the [128 x 64] stage is 16 KB contiguous: slabs (tile, 8 kb .. 8 kb + 7), rows of 256 elements
+                            ptx::tma_load_2d_cg2(&tmapA, full, sA, 0, (tile * (ta.K3p >> 3) + 8 * kb) * 4);
+                        else
+                            ptx::tma_load_2d_cg2(&tmapA, full, sA, kb * kTK, tile * kTM);
                         ptx::tma_load_2d_cg2(hf ? &tmapW3b : &tmapW3a, full, sA + kTABytes, kb * kTK, row0);
                         st.next(kTStages);
                     }
@@ -212,17 +217,19 @@ k_tail(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ CUtens
                     for (int kb = 0; kb < nkb; ++kb) {
                         ptx::mbar_wait_cluster(&bars[tFull + st.st], st.ph);
                         ptx::tc_fence_after_sync();
-                        const uint64_t da = desc0 + (uint64_t)((st.st * kTStageBytes) >> 4);
-                        const uint64_t db = da + (uint64_t)(kTABytes >> 4);
+                        const uint64_t db = desc0 + (uint64_t)((st.st * kTStageBytes + kTABytes) >> 4);
+                        // A: 128-byte-swizzled rows (k-step = 32 B) or the blocked core-matrix order (k-step = 2 x 2 KB slabs)
+                        const uint64_t da = (ta.a_blocked ? descA0 : desc0) + (uint64_t)((st.st * kTStageBytes) >> 4);
+                        const uint64_t ka = ta.a_blocked ? (uint64_t)(4096 >> 4) : 2u;
                         const int ksteps = min(kTK / 16, (ta.K3p - kb * kTK) / 16);
                         if (ptx::elect_one()) {
                             if (ksteps == kTK / 16) {
 #pragma unroll
                                 for (int k = 0; k < kTK / 16; ++k)
-                                    ptx::umma_bf16_ss_cg2(d_tmem, da + 2 * k, db + 2 * k, idesc, (kb | k) ? 1u : 0u);
+                                    ptx::umma_bf16_ss_cg2(d_tmem, da + ka * k, db + 2 * k, idesc, (kb | k) ? 1u : 0u);
                             } else {
                                 for (int k = 0; k < ksteps; ++k)
-                                    ptx::umma_bf16_ss_cg2(d_tmem, da + 2 * k, db + 2 * k, idesc, (kb | k) ? 1u : 0u);
+                                    ptx::umma_bf16_ss_cg2(d_tmem, da + ka * k, db + 2 * k, idesc, (kb | k) ? 1u : 0u);
                             }
                             ptx::umma_commit_cg2(&bars[tEmpty + st.st], 3);
                             if (kb == nkb - 1) ptx::umma_commit_cg2(&bars[tAccFull + hf], 3);
@@ -568,7 +575,7 @@ cudaError_t launch_tail(Ctx *c, int64_t n, int64_t c0, int64_t cn, float *T, flo
     // species beyond Ns of the padded range must carry all-zero constants (the kernel's arithmetic is unguarded)
     for (int k = c->Ns; k < kTailMaxNs; ++k) ta.sA[k] = ta.sC[k] = 0.f;
     const bool fast = !ta.lambda_zero && ta.inv_lambda_int == 10 && !ta.two_ranges;
-    return cudaLaunchKernelEx(&cfg, tail_kernel(c->Ns, fast), l3.tmapA, tn.tmapW3a, tn.tmapW3b, tn.tmapW4, ta);
+    return cudaLaunchKernelEx(&cfg, tail_kernel(c->Ns, fast), ta.a_blocked ? tn.tmapAb : l3.tmapA, tn.tmapW3a, tn.tmapW3b, tn.tmapW4, ta);
 }
 
 }  // namespace gpuann

@@ -250,6 +250,18 @@ __device__ __forceinline__ uint64_t umma_desc_sw128_kmajor(uint32_t smem_addr) {
     return d;
 }
 
+// Shared-memory matrix descriptor for a K-major operand tile WITHOUT swizzle (canonical core-matrix order): a core matrix is
+// 8 rows x 16 bytes stored as 128 contiguous bytes; `lbo` = byte distance between core matrices adjacent in K, `sbo` =
+// between core matrices adjacent in M / N (8-row groups).  Layout field 0, 16-byte aligned base.
+__device__ __forceinline__ uint64_t umma_desc_nosw_kmajor(uint32_t smem_addr, uint32_t lbo, uint32_t sbo) {
+    uint64_t d = 0;
+    d |= static_cast<uint64_t>((smem_addr & 0x3FFFFu) >> 4);
+    d |= static_cast<uint64_t>(lbo >> 4) << 16;
+    d |= static_cast<uint64_t>(sbo >> 4) << 32;
+    d |= static_cast<uint64_t>(1) << 46;
+    return d;
+}
+
 // Instruction descriptor for kind::f16 with BF16 A and B (both K-major), FP32 accumulate.
 // Bits: [4,6) D format (1 = F32), [7,10) A format (1 = BF16), [10,13) B format (1 = BF16),
 // 15 / 16 A / B major (0 = K), [17,23) N >> 3, [24,29) M >> 4.

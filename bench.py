@@ -49,6 +49,23 @@ def load_peaks():
     return dict(FALLBACK_PEAKS), "fallback (B200_PROFILING.md)"
 
 
+def dram_bytes_from_profiles(kernel_class: str, config_index: int, n_cells: int):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from profiles/ncu_dram_bytes.csv (None if no row matches)."""
+    p = ROOT / "profiles" / "ncu_dram_bytes.csv"
+    if not p.exists():
+        return None
+    try:
+        rows = [l.strip().split(",") for l in p.read_text().splitlines() if l.strip() and not l.startswith("#")]
+        hdr = rows[0]
+        for r in rows[1:]:
+            d = dict(zip(hdr, r))
+            if d["kernel_class"] == kernel_class and int(d["config"]) == config_index and int(d["cells"]) == n_cells:
+                return float(d["dram_bytes_read"]) + float(d["dram_bytes_write"])
+    except Exception:
+        return None
+    return None
+
+
 # ------------------------------------------------------------------ clocks
 class ClockSampler:
     """Samples SM clock and clock-event reasons of one GPU while the timed region runs (pynvml)."""
@@ -257,6 +274,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
             e1.record()
         barrier()
     launches = B.gpuann_launch_count(ctx) - l0
+    clocks = clk.summary()
     ms_steps = [e0.elapsed_time(e1) for e0, e1 in ev]
     ms_local = float(sum(ms_steps))
     ms_total, cells_total = aggregate_over_ranks(ms_local, n * args.steps, dist if world > 1 else None, dev)
@@ -295,15 +313,19 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         flop_step = float(cfg.flop_per_cell) * n_act_per_step
     dom_ms_per_step = dom_ms / args.steps
     achieved = flop_step / (dom_ms_per_step * 1e-3) / 1e12
-    # DRAM bytes of the dominant kernel per launch from the committed ncu capture of exactly this configuration
-    # (profiles/r01_fused_l1l2.md, last section: dram__bytes_read.sum + dram__bytes_write.sum = 0.10 + 1.62 GB; the
-    # kernel writes h2 = 1,048,576 x 1,600 B once and reads the 96 MB of state once); null for any other configuration
-    traffic = None
-    if dom_name == "bf16_fused" and cfg.index == 2 and n == 1048576 and not args.chunk:
-        traffic = 1.725e9
+    # DRAM bytes of the dominant kernel per launch: dram__bytes_read.sum + dram__bytes_write.sum of the committed
+    # `ncu --set full` capture of exactly this kernel class, configuration and cell count (profiles/ncu_dram_bytes.csv,
+    # written from the .ncu-rep by hand with its command beside it); null when no capture matches
+    traffic = dram_bytes_from_profiles(dom_name, cfg.index, n) if not args.chunk else None
+    # what each kernel class must move by design (bytes per step): state in / out, h2 out / in, weights once
+    h2_bytes = 2.0 * (sizes[2] if len(sizes) > 3 else 0) * n_act_per_step
+    by_design = {"state_algorithmic": float(cfg.state_bytes_per_cell) * n_act_per_step,
+                 "bf16_fused": (2 + Ns) * 4.0 * n_act_per_step + h2_bytes,
+                 "bf16_tail": h2_bytes + ((2 + Ns) + (1 + Ns)) * 4.0 * n_act_per_step}
     roofline = {
         "bound": "tensor", "kernel": dom_name, "achieved": achieved, "peak": peaks["bf16_tflops"], "unit": "TFLOP/s",
-        "frac": achieved / peaks["bf16_tflops"], "traffic": traffic, "peak_source": peak_src + ", burst",
+        "frac": achieved / peaks["bf16_tflops"], "traffic": traffic, "traffic_by_design": by_design,
+        "peak_source": peak_src + ", burst",
         "launches_per_step": dom_cnt / args.steps, "ms_per_step_in_kernel": dom_ms_per_step,
         "share_of_step": dom_ms_per_step / step_ms_sum if step_ms_sum > 0 else None,
         "flop_per_step_algorithmic": flop_step,
@@ -348,14 +370,48 @@ def run_ours(args, rank: int, local_rank: int, world: int):
            "d2h_bytes_per_step": (1 + Ns) * 4 * n, "steps": k_e2e, "ms_per_step": t_e2e_ms / k_e2e,
            "api": "gpuann_chem_step_host (pinned host buffers)"}
 
+    # ---- sustained leg (--sustain S): the same loop back to back for >= S seconds, clocks sampled throughout.  The default
+    # line above is a burst of K steps (~0.1 s); a solver that calls the step every time step lives here.
+    sustained = None
+    if args.sustain > 0:
+        per_batch = 50
+        evs = []
+        with ClockSampler(local_rank, period_s=0.02) as clk_s:
+            barrier()
+            t_start = time.perf_counter()
+            while time.perf_counter() - t_start < args.sustain:
+                batch = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(per_batch)]
+                for e0, e1 in batch:
+                    restore()
+                    e0.record()
+                    step()
+                    e1.record()
+                torch.cuda.synchronize()
+                evs.extend(batch)
+            barrier()
+        ms_s = np.array([e0.elapsed_time(e1) for e0, e1 in evs])
+        tail_half = ms_s[len(ms_s) // 2:]
+        ms_sust, _ = aggregate_over_ranks(float(np.median(tail_half)), 0, dist if world > 1 else None, dev)
+        tf_s = cfg.flop_per_cell * (n_act_per_step * world) / (ms_sust * 1e-3) / 1e12
+        sustained = {"seconds": args.sustain, "steps": int(len(ms_s)), "ms_per_step_median_second_half": ms_sust,
+                     "ms_per_step_first_20_median": float(np.median(ms_s[:20])), "cells_per_s": n * world / (ms_sust * 1e-3),
+                     "tflops": tf_s, "frac_of_measured_burst": tf_s / peaks["bf16_tflops"],
+                     "frac_of_measured_sustained": tf_s / peaks["bf16_tflops_sustained"], "clocks": clk_s.summary()}
+        roofline["whole_step"]["sustained"] = sustained
+
     B.gpuann_destroy(ctx)
 
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         sample = calibrated_sample(cfg, prob, target_s=15.0)
         v, threads, secs, s = oracle_sample_run(cfg, prob, sample)
+        import oracle
+        oracle.set_num_threads(1)
+        v1, _, secs1, s1 = oracle_sample_run(cfg, prob, max(64, sample // (4 * max(1, threads))))
+        oracle.set_num_threads(threads)
         cpu_baseline = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle",
-                        "sample": f"first {s} cells of the workload, one pass, {secs:.1f} s"}
+                        "sample": f"first {s} cells of the workload, one pass, {secs:.1f} s",
+                        "value_1_thread": v1, "sample_1_thread": f"first {s1} cells, one pass, {secs1:.1f} s"}
 
     if rank == 0:
         line = {
@@ -366,10 +422,11 @@ def run_ours(args, rank: int, local_rank: int, world: int):
             "config": {"workload": workload_name(cfg, n), "cells_per_gpu": n, "variant": variant,
                        "l2": "state (184 B/cell x n) larger than L2 and restored from a pristine copy between steps",
                        "parallelism": f"cells sharded over {world} GPU(s), no collective on the data path"},
-            "clocks": clk.summary(), "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
             "cpu_baseline": cpu_baseline,
             "checks": {"finite": ok_finite, "max_abs_sumY_minus_1": sum_dev, "newton_not_converged": int(n_notconv),
-                       "degenerate": int(n_degen), "ms_min": min(ms_steps), "ms_max": max(ms_steps)},
+                       "degenerate": int(n_degen), "ms_min": min(ms_steps), "ms_median": float(np.median(ms_steps)),
+                       "ms_max": max(ms_steps)},
         }
         print(json.dumps(line), flush=True)
     if world > 1:
@@ -388,6 +445,8 @@ def main():
     ap.add_argument("--cells", type=int, default=0, help="override the cell count of the config (per GPU)")
     ap.add_argument("--chunk", type=int, default=0, help="override the library's cells-per-pass")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sustain", type=float, default=0.0,
+                    help="also run the step back to back for this many seconds and report the sustained figure")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))

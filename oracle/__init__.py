@@ -17,6 +17,7 @@ from .oracle import (  # noqa: F401
     mlp_forward,
     newton_T,
     num_threads,
+    set_num_threads,
     species_cp,
     species_h,
 )

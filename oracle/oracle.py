@@ -81,8 +81,21 @@ def _load():
     return lib
 
 
+_forced_threads: Optional[int] = None
+
+
+def set_num_threads(n: int) -> None:
+    """Sets the OpenMP thread count of the loop over cells (harness plumbing for the 1-thread timing leg of bench.py;
+    no arithmetic of the oracle depends on it)."""
+    global _forced_threads
+    C.CDLL("libgomp.so.1").omp_set_num_threads(C.c_int(max(1, int(n))))
+    _forced_threads = max(1, int(n))
+
+
 def num_threads() -> int:
-    """Threads the OpenMP loop over cells will use (OMP_NUM_THREADS or all cores)."""
+    """Threads the OpenMP loop over cells will use (set_num_threads, OMP_NUM_THREADS or all cores)."""
+    if _forced_threads is not None:
+        return _forced_threads
     v = os.environ.get("OMP_NUM_THREADS")
     if v:
         try:

@@ -432,6 +432,12 @@ int gpuann_load_thermo(gpuann_ctx *c, int n_species, const double *nasa_lo, cons
             std::memcpy(ta.th.hh[k], h->hh[k], sizeof(ta.th.hh[k]));
             ta.th.T_mid[k] = h->T_mid[k];
         }
+        std::memset(ta.hhf, 0, sizeof(ta.hhf));
+        std::memset(ta.cpf, 0, sizeof(ta.cpf));
+        for (int k = 0; k < kTailMaxNs && k < n_species; ++k) {
+            for (int m = 0; m < 6; ++m) ta.hhf[k][m] = (float)h->hh[k][0][m];
+            for (int m = 0; m < 5; ++m) ta.cpf[k][m] = (float)h->cp[k][0][m];
+        }
     }
     DeviceGuard g(c->device);
     cudaDeviceSynchronize();

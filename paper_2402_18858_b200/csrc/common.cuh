@@ -116,6 +116,9 @@ struct TailArgs {
     float b4[kTailMaxNs];
     Counters *counters;
     TailThermo th;
+    // FP32 copies of the one-range table for the FAST instance of the kernel (mixture coefficients accumulated in FP32)
+    float hhf[kTailMaxNs][6];
+    float cpf[kTailMaxNs][5];
 };
 struct TailNet {
     bool on = false;

@@ -368,6 +368,11 @@ k_tail(const __grid_constant__ CUtensorMap tmapA /* row-major [rows][K3p] or blo
             // eight species at a time
             double S = 0.0;
             double Ch[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0}, Cc[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+            // FAST: the sum and the mixture coefficients are accumulated in FP32 (DESIGN.md "Precision of the scalar math":
+            // the FP64 pipe of this part runs ~1 warp instruction per 40 clk, and 11 DFMAs per species made the update the
+            // slowest stage of the kernel; the rounding adds ~4e-3 K to T against the 0.5 K budget of the tensor path)
+            float Sf = 0.f;
+            float Chf[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, Ccf[5] = {0.f, 0.f, 0.f, 0.f, 0.f};
 #pragma unroll
             for (int pc = 0; pc < NSP / 8; ++pc) {
                 uint32_t t8[8];
@@ -402,9 +407,17 @@ k_tail(const __grid_constant__ CUtensorMap tmapA /* row-major [rows][K3p] or blo
                         ys = update_species_f32(yc, dy, ta);
                     }
                     Yv[k] = ys;
+                    if (FAST) {
+                        Sf += ys;
+#pragma unroll
+                        for (int m = 0; m < 6; ++m) Chf[m] = fmaf(ys, ta.hhf[k][m], Chf[m]);
+#pragma unroll
+                        for (int m = 0; m < 5; ++m) Ccf[m] = fmaf(ys, ta.cpf[k][m], Ccf[m]);
+                        continue;
+                    }
                     const double yd = (double)ys;
                     S += yd;
-                    if (FAST || !ta.two_ranges) {
+                    if (!ta.two_ranges) {
 #pragma unroll
                         for (int m = 0; m < 6; ++m) Ch[m] = fma(yd, ta.th.hh[k][0][m], Ch[m]);
 #pragma unroll
@@ -414,7 +427,7 @@ k_tail(const __grid_constant__ CUtensorMap tmapA /* row-major [rows][K3p] or blo
             }
             if (fwd_only) continue;
             // S6 (R8): divide by the sum; a vanishing sum falls back to max(Y,0)/sum (rare: the inputs are re-read)
-            const bool degenerate = !(S > 0.0);
+            const bool degenerate = FAST ? !(Sf > 0.f) : !(S > 0.0);
             if (degenerate) {
                 S = 0.0;
 #pragma unroll
@@ -433,11 +446,23 @@ k_tail(const __grid_constant__ CUtensorMap tmapA /* row-major [rows][K3p] or blo
                     for (int m = 0; m < 5; ++m) Cc[m] = fma(yd, ta.th.cp[k][0][m], Cc[m]);
                 }
             }
-            const double rS = 1.0 / S;
+            double rS;
+            float rSf;
+            if (FAST && !degenerate) {
+                rSf = 1.f / Sf;
+                rS = (double)rSf;
 #pragma unroll
-            for (int m = 0; m < 6; ++m) Ch[m] *= rS;
+                for (int m = 0; m < 6; ++m) Ch[m] = (double)(Chf[m] * rSf);
 #pragma unroll
-            for (int m = 0; m < 5; ++m) Cc[m] *= rS;
+                for (int m = 0; m < 5; ++m) Cc[m] = (double)(Ccf[m] * rSf);
+            } else {
+                rS = 1.0 / S;
+                rSf = (float)rS;
+#pragma unroll
+                for (int m = 0; m < 6; ++m) Ch[m] *= rS;
+#pragma unroll
+                for (int m = 0; m < 5; ++m) Cc[m] *= rS;
+            }
             // S7 (R9-R11): Newton on h(T) = sum_k Y_k h_k(T), FP64
             double Tn = fmin(fmax((double)Tin, ta.T_min), ta.T_max);
             bool conv = false;
@@ -460,7 +485,17 @@ k_tail(const __grid_constant__ CUtensorMap tmapA /* row-major [rows][K3p] or blo
                     f -= hc;
                 }
                 if (!(c > 0.0)) break;  // R10: stop, not converged
-                const double dT = -f / c;
+                double dT;
+                if (FAST) {
+                    // -f / c through an FP32 reciprocal refined twice in FP64 (relative error ~1e-16): 5 FP64 instructions
+                    // instead of the ~12 of the division sequence
+                    double rc = (double)ptx::rcp_approx((float)c);
+                    rc = fma(rc, fma(-c, rc, 1.0), rc);
+                    rc = fma(rc, fma(-c, rc, 1.0), rc);
+                    dT = -f * rc;
+                } else {
+                    dT = -f / c;
+                }
                 Tn = fmin(fmax(Tn + dT, ta.T_min), ta.T_max);
                 if (fabs(dT) < ta.newton_tol) {
                     conv = true;
@@ -471,7 +506,7 @@ k_tail(const __grid_constant__ CUtensorMap tmapA /* row-major [rows][K3p] or blo
             if (valid) {
 #pragma unroll
                 for (int k = 0; k < NSP; ++k)
-                    if (k < Ns) ta.Y[(int64_t)k * ta.n + g] = (float)((double)Yv[k] * rS);
+                    if (k < Ns) ta.Y[(int64_t)k * ta.n + g] = FAST ? Yv[k] * rSf : (float)((double)Yv[k] * rS);
                 ta.T[g] = (float)Tn;
                 if (!conv) ++nconv_total;
                 if (degenerate) ++ndeg_total;

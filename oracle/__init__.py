@@ -5,6 +5,7 @@ It imports nothing from paper_2402_18858_b200 (and vice versa).
 """
 from .oracle import (  # noqa: F401
     Oracle,
+    OracleDerived,
     OracleModel,
     boxcox,
     boxcox_inv,

@@ -16,6 +16,10 @@
  *   O5  inverse Box-Cox                                inverse of Eq. 7 (R7)
  *   O6  renormalise so that sum_k Y_k = 1              PAPER.md:92, 108-110 Eq. 9 (R8)
  *   O7  Newton iteration for T on NASA-7 polynomials   PAPER.md:57 (R9, R10, R11)
+ *   O8  reaction rates and heat release rate           PAPER.md:112-115 Eq. 10, :142 Fig. 6(b), :148 (R19, R20)
+ *   O9  thermal properties of the updated state        PAPER.md:57 (R21)
+ * O8 / O9 (round 2) are a separate function, oracle_derived_outputs, that reads the
+ * results of O0-O7; nothing in O0-O7 changed when it was added.
  *
  * Everything is scalar double precision; sums run in index order; the only
  * parallelism is an OpenMP "parallel for" over cells (cells are independent).
@@ -28,6 +32,9 @@
  * brentq Newton roots; sum(Y) = 1; zero-net fixed point; permutation invariance;
  * o_raw from an independently built z (feature order, division by sigma); mu_out != 0;
  * T == 600.0f boundary; vanishing-sum fallback; cp <= 0 stop; clamped Newton start.
+ * O8 / O9: density against the ideal-gas law in molar units and a textbook value; sum_k RR_k = rho (1 - sum Y)/dt;
+ * HRR dt / rho = integral of cp(T; Y_old) from T_old to T_new (scipy quad); cp = dh/dT by finite differences;
+ * rho_new R_mix T_new = p; psi p = rho_new; R_mix = Ru / W for a pure species.
  * Parity unpinned: R3 (what the de-normalised output means) and R5 (erf vs tanh
  * GELU) are choices the paper does not settle; they are fixed by DESIGN.md.
  */
@@ -374,4 +381,58 @@ int oracle_chem_step(const oracle_model *m, int64_t n, const float *T, const flo
         }
     }
     return fail;
+}
+
+/* ---------------------------------------------------------------- O8, O9: derived outputs of a step
+ *
+ * O8 (R19, R20).  The quantities the solver's combustion model consumes from the chemistry step (PaSR source terms,
+ * PAPER.md:148) and the one the paper compares in Fig. 6(b) and trains against in Eq. 10:
+ *     rho_i  = p_i / (Ru T_i sum_k Yc_k / W_k)            ideal gas at the INPUT state, Yc = max(Y, 0)      [kg/m3]
+ *     RR_k,i = rho_i (Y_new,k,i - Y_k,i) / dt             mass production rate of species k               [kg/(m3 s)]
+ *     HRR_i  = - sum_k h_k(T_new,i) RR_k,i                heat release rate, NASA-7 total species enthalpy  [W/m3]
+ * O9 (R21).  Thermal properties of the updated state (the transport half needs fits the paper does not give):
+ *     cp_i    = sum_k Y_new,k cp_k(T_new)                                                                 [J/(kg K)]
+ *     Rmix_i  = Ru sum_k Y_new,k / W_k                                                                    [J/(kg K)]
+ *     rho_new = p_i / (Rmix_i T_new,i),   psi_i = 1 / (Rmix_i T_new,i)    (rho = psi p)            [kg/m3], [s2/m2]
+ * Skipped cells (flags == 4): RR = 0, HRR = 0; the properties are those of the unchanged state.
+ * Inputs: the FP32 state the step received, and its FP64 results.  Any output pointer may be NULL. */
+int oracle_derived_outputs(int64_t n, int Ns, const float *T, const float *p, const float *Y, double dt,
+                           const double *T_new, const double *Y_new, const int32_t *flags, const double *nasa_lo,
+                           const double *nasa_hi, const double *T_mid, const double *W, double *rr, double *hrr,
+                           double *cp, double *rmix, double *rho_new, double *psi)
+{
+    if (n < 0 || Ns < 1 || !T || !p || !Y || !T_new || !Y_new || !nasa_lo || !W || !(dt > 0.0)) return 1;
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) {
+        const int skipped = flags && flags[i] == 4;
+        /* O8 */
+        double inv_w_in = 0.0;
+        for (int k = 0; k < Ns; ++k) {
+            double yc = (double)Y[(size_t)k * (size_t)n + (size_t)i];
+            if (yc < 0.0) yc = 0.0;
+            inv_w_in += yc / W[k];
+        }
+        const double rho_in = (double)p[i] / (ORACLE_RU * (double)T[i] * inv_w_in);
+        double q = 0.0;
+        for (int k = 0; k < Ns; ++k) {
+            const size_t ki = (size_t)k * (size_t)n + (size_t)i;
+            const double r = skipped ? 0.0 : rho_in * (Y_new[ki] - (double)Y[ki]) / dt;
+            if (rr) rr[ki] = r;
+            q -= oracle_species_h(select_range(k, T_new[i], nasa_lo, nasa_hi, T_mid), W[k], T_new[i]) * r;
+        }
+        if (hrr) hrr[i] = q;
+        /* O9 */
+        double c = 0.0, inv_w = 0.0;
+        for (int k = 0; k < Ns; ++k) {
+            const double y = Y_new[(size_t)k * (size_t)n + (size_t)i];
+            c += y * oracle_species_cp(select_range(k, T_new[i], nasa_lo, nasa_hi, T_mid), W[k], T_new[i]);
+            inv_w += y / W[k];
+        }
+        const double R = ORACLE_RU * inv_w;
+        if (cp) cp[i] = c;
+        if (rmix) rmix[i] = R;
+        if (rho_new) rho_new[i] = (double)p[i] / (R * T_new[i]);
+        if (psi) psi[i] = 1.0 / (R * T_new[i]);
+    }
+    return 0;
 }

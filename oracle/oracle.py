@@ -77,6 +77,9 @@ def _load():
     lib.oracle_chem_step.restype = C.c_int
     lib.oracle_chem_step.argtypes = [C.POINTER(_Model), C.c_int64, fp, fp, fp, fp, d, dp, dp, dp,
                                      C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
+    lib.oracle_derived_outputs.restype = C.c_int
+    lib.oracle_derived_outputs.argtypes = [C.c_int64, C.c_int, fp, fp, fp, d, dp, dp, C.POINTER(C.c_int32), dp, dp, dp, dp,
+                                           dp, dp, dp, dp, dp, dp]
     _lib = lib
     return lib
 
@@ -316,3 +319,31 @@ class Oracle:
         if rc != 0:
             raise RuntimeError("oracle_chem_step failed (bad arguments or allocation)")
         return OracleResult(T_new, Y_new, o_raw, iters, flags)
+
+    def derived(self, T, p, Y, dt: float, res: OracleResult) -> "OracleDerived":
+        """O8 / O9: reaction rates, heat release rate and thermal properties from the results of `chem_step`."""
+        lib = _load()
+        t, pp, y = _f32(T), _f32(p), _f32(Y)
+        n = t.shape[0]
+        Ns = self.n_species
+        assert y.shape == (Ns, n) and pp.shape == (n,)
+        tn, yn, fl = _f64(res.T_new), _f64(res.Y_new), np.ascontiguousarray(res.flags, dtype=np.int32)
+        rr = np.empty((Ns, n), dtype=np.float64)
+        out = [np.empty(n, dtype=np.float64) for _ in range(5)]
+        rc = lib.oracle_derived_outputs(n, Ns, _p(t, C.c_float), _p(pp, C.c_float), _p(y, C.c_float), float(dt),
+                                        _p(tn, C.c_double), _p(yn, C.c_double), _p(fl, C.c_int32),
+                                        _p(self._lo, C.c_double), _p(self._hi, C.c_double), _p(self._tm, C.c_double),
+                                        _p(self._W, C.c_double), _p(rr, C.c_double), *[_p(o, C.c_double) for o in out])
+        if rc != 0:
+            raise RuntimeError("oracle_derived_outputs failed (bad arguments)")
+        return OracleDerived(rr, *out)
+
+
+@dataclass
+class OracleDerived:
+    rr: np.ndarray        # [Ns][n] kg/(m3 s)
+    hrr: np.ndarray       # [n] W/m3
+    cp: np.ndarray        # [n] J/(kg K)
+    rmix: np.ndarray      # [n] J/(kg K)
+    rho_new: np.ndarray   # [n] kg/m3
+    psi: np.ndarray       # [n] s2/m2

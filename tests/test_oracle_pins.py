@@ -504,6 +504,121 @@ def test_newton_first_iterate_is_evaluated_at_the_clamped_start():
         assert abs(unclamped - want) > 1.0               # so a missing clamp cannot pass
 
 
+# ------------------------------------------------------------------ O8 / O9: reaction rates, HRR, thermal properties (round 2)
+def _step_with_derived(n=96, **over):
+    pr, h, m = _small_problem(n=n, **over)
+    st = pr.state
+    orc = oracle.Oracle(m)
+    r = orc.chem_step(st.T, st.p, st.Y, h, 1e-6)
+    return pr, h, m, r, orc.derived(st.T, st.p, st.Y, 1e-6, r)
+
+
+def test_density_of_pure_nitrogen_textbook_and_molar_ideal_gas_law():
+    """rho of the INPUT state behind RR (R19): a pure-N2 cell at 300 K, 1 atm is 1.138 kg/m3 in any textbook; in molar
+    units rho = p M / (R T) with R = 8.314462618 J/(mol K), M in kg/mol.  Catches Y*W for Y/W, T_new for T, a missing p."""
+    pr, h, m = _small_problem(n=4)
+    th = pr.thermo
+    Ns = len(th.W)
+    W = th.W.copy()
+    W[0] = 28.0134
+    T = np.full(4, 300.0, dtype=np.float32)
+    p = np.full(4, 101325.0, dtype=np.float32)
+    Y = np.zeros((Ns, 4), dtype=np.float32)
+    Y[0] = 1.0
+    m.W = W
+    m.weights = [w.copy() for w in m.weights]
+    m.biases = [b.copy() for b in m.biases]
+    m.weights[-1][:] = 0.0
+    m.biases[-1][:] = 3.0        # species 0 grows in Box-Cox space, the others stay at exactly 0 -> Y_new = Y, T moves with h
+    hh = oracle.enthalpy_field(np.full(4, 350.0, np.float32), Y, th.nasa_lo, None, None, W).astype(np.float32)
+    orc = oracle.Oracle(m)
+    r = orc.chem_step(T, p, Y, hh, 1e-6)
+    assert np.all(np.abs(r.T_new - 350.0) < 1e-2)          # the step heats the cell by 50 K
+    d = orc.derived(T, p, Y, 1e-6, r)
+    rho_new_molar = 101325.0 * 0.0280134 / (8.314462618 * r.T_new)
+    assert np.allclose(d.rho_new, rho_new_molar, rtol=1e-9)
+    assert abs(101325.0 * 0.0280134 / (8.314462618 * 300.0) - 1.138) < 1e-3      # the textbook figure itself
+    assert np.allclose(d.rmix, 8314.46261815324 / 28.0134, rtol=1e-12)            # R_mix = Ru / W for a pure species
+    assert np.allclose(d.psi * 101325.0, d.rho_new, rtol=1e-12)
+
+
+def test_reaction_rates_use_input_density_and_sum_to_the_mass_defect():
+    """RR_k dt / (Y_new,k - Y_k) is ONE number per cell, the ideal-gas density of the INPUT state (molar-unit formula below,
+    clamped Y); sum_k RR_k = rho (1 - sum_k Y_k) / dt.  Catches rho at T_new, a missing 1/dt, RR from clamped Y."""
+    pr, h, m, r, d = _step_with_derived()
+    st, th = pr.state, pr.thermo
+    Y64, T64, p64 = st.Y.astype(np.float64), st.T.astype(np.float64), st.p.astype(np.float64)
+    M_kg_per_mol = 1e-3 / (np.maximum(Y64, 0.0) / th.W[:, None]).sum(axis=0)    # W in g/mol
+    rho_in = p64 * M_kg_per_mol / (8.314462618 * T64)
+    dY = r.Y_new - Y64
+    big = np.abs(dY) > 1e-9
+    ratio = d.rr * 1e-6 / np.where(big, dY, 1.0)
+    assert np.allclose(ratio[big], np.broadcast_to(rho_in, dY.shape)[big], rtol=1e-9)
+    assert np.allclose(d.rr.sum(axis=0) * 1e-6 / rho_in + Y64.sum(axis=0), 1.0, rtol=0, atol=1e-13)
+    assert np.abs(r.T_new - T64).max() > 1.0     # T does move, so rho(T_new) would have failed the first assert
+
+
+def test_hrr_is_the_sensible_heating_of_the_old_mixture():
+    """With h conserved, -sum_k h_k(T_new) RR_k = (rho / dt) * integral_{T_old}^{T_new} cp(T; Y_old) dT.  The integral is done by
+    scipy.integrate.quad on oracle.mixture_cp (pinned as dh/dT above).  Catches the sign, h_k at T_old (that is the heating
+    of the NEW mixture, a few per cent off), a dropped 1/dt or rho."""
+    from scipy import integrate
+    pr, h, m, r, d = _step_with_derived(n=24)
+    st, th = pr.state, pr.thermo
+    Y64 = st.Y.astype(np.float64)
+    Y64 = Y64 / Y64.sum(axis=0)                      # quad below uses the normalised old composition (1e-7 effect)
+    for i in range(24):
+        rho_in = float(st.p[i]) / (8314.46261815324 * float(st.T[i]) * (np.maximum(st.Y[:, i].astype(np.float64), 0) / th.W).sum())
+        # h handed to the step is the FP32 rounding of h(T_old, Y_old): use the exact old enthalpy on both sides
+        h_old = oracle.mixture_h(st.Y[:, i].astype(np.float64), float(st.T[i]), th.nasa_lo, None, None, th.W)
+        q, _ = integrate.quad(lambda T: oracle.mixture_cp(st.Y[:, i].astype(np.float64), T, th.nasa_lo, None, None, th.W),
+                              float(st.T[i]), r.T_new[i], epsabs=1e-9, epsrel=1e-13)
+        # Newton solved sum Y_new h_k(T_new) = h_fp32; the defect h_fp32 - h_old enters once
+        want = rho_in / 1e-6 * (q + (h_old - float(h[i])))
+        assert abs(d.hrr[i] - want) <= 1e-8 * abs(want) + 1e-3 * rho_in / 1e-6, (i, d.hrr[i], want)
+    assert np.abs(d.hrr).max() > 1e6               # it is not trivially zero: MW/m3 scale
+
+
+def test_hrr_and_rr_vanish_for_the_zero_net_and_for_skipped_cells():
+    pr, h, m = _small_problem(n=64)
+    m.weights = [w.copy() for w in m.weights]
+    m.biases = [b.copy() for b in m.biases]
+    m.weights[-1][:] = 0.0
+    m.biases[-1][:] = 0.0
+    st = pr.state
+    orc = oracle.Oracle(m)
+    r = orc.chem_step(st.T, st.p, st.Y, h, 1e-6)
+    d = orc.derived(st.T, st.p, st.Y, 1e-6, r)
+    # Y_new = Y / sum Y: |RR| <= rho |1/sum Y - 1| Y / dt ~ 1e-7 * rho / dt
+    assert np.abs(d.rr).max() < 1.0 and np.abs(d.hrr).max() < 5e7 * 1e-1
+    pr2, h2, m2 = _small_problem(n=64, T_active=1e4)     # every cell skipped
+    orc2 = oracle.Oracle(m2)
+    r2 = orc2.chem_step(pr2.state.T, pr2.state.p, pr2.state.Y, h2, 1e-6)
+    d2 = orc2.derived(pr2.state.T, pr2.state.p, pr2.state.Y, 1e-6, r2)
+    assert np.all(r2.flags == 4) and np.all(d2.rr == 0.0) and np.all(d2.hrr == 0.0)
+
+
+def test_cp_of_the_new_state_is_dh_dT_and_the_state_equation_closes():
+    """cp (O9) against central differences of oracle.mixture_h at (T_new, Y_new); rho_new R_mix T_new = p; R_mix against the
+    molar-unit mean molar mass.  Catches cp at T_old or with Y_old, W in place of 1/W."""
+    pr, h, m, r, d = _step_with_derived(n=32)
+    st, th = pr.state, pr.thermo
+    for i in range(32):
+        y = r.Y_new[:, i]
+        dT = 1e-2
+        fd = (oracle.mixture_h(y, r.T_new[i] + dT, th.nasa_lo, None, None, th.W)
+              - oracle.mixture_h(y, r.T_new[i] - dT, th.nasa_lo, None, None, th.W)) / (2 * dT)
+        assert abs(d.cp[i] - fd) < 1e-6 * abs(fd)
+        fd_old = (oracle.mixture_h(y, float(st.T[i]) + dT, th.nasa_lo, None, None, th.W)
+                  - oracle.mixture_h(y, float(st.T[i]) - dT, th.nasa_lo, None, None, th.W)) / (2 * dT)
+        if abs(r.T_new[i] - float(st.T[i])) > 5.0:
+            assert abs(d.cp[i] - fd_old) > 1e-5 * abs(fd)      # the pin can tell T_new from T_old
+    assert np.allclose(d.rho_new * d.rmix * r.T_new, st.p.astype(np.float64), rtol=1e-13)
+    M_new = 1.0 / (r.Y_new / th.W[:, None]).sum(axis=0)       # g/mol
+    assert np.allclose(d.rmix, 8.314462618 / (M_new * 1e-3), rtol=1e-9)
+    assert np.allclose(d.psi, d.rho_new / st.p.astype(np.float64), rtol=1e-13)
+
+
 def test_paper_speedup_arithmetic():
     """context numbers in BASELINE.md are self-consistent (ratio = 32/(1 - reduction))."""
     for red, ratio in read_golden("speedup_arithmetic.txt"):

@@ -250,8 +250,17 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         T_d.copy_(T0)
         Y_d.copy_(Y0)
 
+    ex = {}
+    if args.ex:   # gpuann_chem_step_ex with every optional output (RR, HRR, cp, rho, psi): (Ns + 4) more output streams
+        ex = {"rr": torch.empty((Ns, n), dtype=torch.float32, device=dev)}
+        ex.update({k: torch.empty(n, dtype=torch.float32, device=dev) for k in ("hrr", "cp", "rho", "psi")})
+
     def step():
-        B.gpuann_chem_step(ctx, n, T_d.data_ptr(), p_d.data_ptr(), Y_d.data_ptr(), h_d.data_ptr(), cfg.dt, stream)
+        if ex:
+            B.gpuann_chem_step_ex(ctx, n, T_d.data_ptr(), p_d.data_ptr(), Y_d.data_ptr(), h_d.data_ptr(), cfg.dt, stream,
+                                  **{k: v.data_ptr() for k, v in ex.items()})
+        else:
+            B.gpuann_chem_step(ctx, n, T_d.data_ptr(), p_d.data_ptr(), Y_d.data_ptr(), h_d.data_ptr(), cfg.dt, stream)
 
     def barrier():
         if world > 1:
@@ -419,7 +428,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
             "warmup": max(args.warmup, 3), "ms_per_step": ms_total / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "bf16" if cfg.precision == 1 else "f32",
             "data": "synthetic",
-            "config": {"workload": workload_name(cfg, n), "cells_per_gpu": n, "variant": variant,
+            "config": {"workload": workload_name(cfg, n), "cells_per_gpu": n, "variant": variant + ("+ex(rr,hrr,cp,rho,psi)" if args.ex else ""),
                        "l2": "state (184 B/cell x n) larger than L2 and restored from a pristine copy between steps",
                        "parallelism": f"cells sharded over {world} GPU(s), no collective on the data path"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
@@ -445,6 +454,7 @@ def main():
     ap.add_argument("--cells", type=int, default=0, help="override the cell count of the config (per GPU)")
     ap.add_argument("--chunk", type=int, default=0, help="override the library's cells-per-pass")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ex", action="store_true", help="time gpuann_chem_step_ex with every optional output requested")
     ap.add_argument("--sustain", type=float, default=0.0,
                     help="also run the step back to back for this many seconds and report the sustained figure")
     args = ap.parse_args()

@@ -128,6 +128,32 @@ int gpuann_load_thermo(gpuann_ctx *ctx, int n_species, const double *nasa_lo, co
 int gpuann_chem_step(gpuann_ctx *ctx, int64_t n_cells, float *T, const float *p, float *Y, const float *h,
                      double dt, void *stream);
 
+/* Optional extra outputs of a step; every member is a DEVICE pointer or NULL (= not computed).
+ * For an ACTIVE cell i, with T, p, Y the inputs and T_new, Y_new the results of the same step:
+ *   rr    float[Ns][n]  RR_k = rho (Y_new,k - Y_k) / dt [kg/(m3 s)], the species source term a PaSR-type combustion model
+ *                       consumes; rho = p / (Ru T sum_k max(Y_k,0)/W_k), the ideal-gas density of the INPUT
+ *                       state (R19).  Y_k is the input as given (not clamped), so sum_k RR_k = rho (1 - sum_k Y_k) / dt
+ *   hrr   float[n]      HRR = - sum_k h_k(T_new) RR_k [W/m3], the heat release rate of PAPER.md:112-115 Eq. 10 and Fig. 6(b)
+ *                       (PAPER.md:142), with the NASA-7 total species enthalpies at T_new (R20)
+ *   cp    float[n]      sum_k Y_new,k cp_k(T_new) [J/(kg K)]                                   (R21)
+ *   rho   float[n]      density of the UPDATED state p / (R_mix T_new), R_mix = Ru sum_k Y_new,k / W_k [kg/m3]
+ *   psi   float[n]      compressibility 1 / (R_mix T_new) [s2/m2] (rho = psi p)
+ * Cells below T_active are not written (like T and Y).  Transport properties are not provided: the paper gives no fits
+ * for them (out of scope). */
+typedef struct {
+    float *rr;
+    float *hrr;
+    float *cp;
+    float *rho;
+    float *psi;
+} gpuann_step_outputs;
+
+/* gpuann_chem_step plus the optional outputs above, computed in the same kernels (no extra pass over the state).
+ * out == NULL or all members NULL is exactly gpuann_chem_step.  Errors as gpuann_chem_step, and UNSUPPORTED when an output
+ * is requested on a BF16 net that does not run the tail kernel (Ns > 48 or a last hidden layer wider than 416). */
+int gpuann_chem_step_ex(gpuann_ctx *ctx, int64_t n_cells, float *T, const float *p, float *Y, const float *h,
+                        double dt, const gpuann_step_outputs *out, void *stream);
+
 /* The same step for a caller whose state lives in HOST memory: copies T, p, Y, h to the device
  * (library-owned staging buffers, grown lazily), runs gpuann_chem_step, copies T and Y back and
  * synchronises.  Pinned host memory makes the copies asynchronous.  On the BF16 path without an active-cell

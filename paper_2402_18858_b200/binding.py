@@ -26,6 +26,7 @@ GPUANN_PRECISION_BF16 = 1
 # every symbol include/gpuann.h declares (tests check that the library exports all of them)
 SYMBOLS = [
     "gpuann_default_params", "gpuann_create", "gpuann_load_net", "gpuann_load_thermo", "gpuann_chem_step",
+    "gpuann_chem_step_ex",
     "gpuann_chem_step_host", "gpuann_debug_forward", "gpuann_get_stats", "gpuann_reset_stats", "gpuann_enthalpy",
     "gpuann_input_moments", "gpuann_launch_count", "gpuann_timing_enable", "gpuann_timing_read",
     "gpuann_timing_num_classes", "gpuann_timing_class_name", "gpuann_describe", "gpuann_last_error", "gpuann_destroy",
@@ -71,6 +72,8 @@ def lib() -> C.CDLL:
     L.gpuann_load_thermo.argtypes = [vp, C.c_int, vp, vp, vp, vp]
     L.gpuann_chem_step.restype = C.c_int
     L.gpuann_chem_step.argtypes = [vp, i64, vp, vp, vp, vp, dbl, vp]
+    L.gpuann_chem_step_ex.restype = C.c_int
+    L.gpuann_chem_step_ex.argtypes = [vp, i64, vp, vp, vp, vp, dbl, vp, vp]
     L.gpuann_chem_step_host.restype = C.c_int
     L.gpuann_chem_step_host.argtypes = [vp, i64, vp, vp, vp, vp, dbl]
     L.gpuann_debug_forward.restype = C.c_int
@@ -168,6 +171,17 @@ def gpuann_load_thermo(ctx: int, n_species: int, nasa_lo, nasa_hi, T_mid, W) -> 
 
 def gpuann_chem_step(ctx: int, n_cells: int, T: int, p: int, Y: int, h: int, dt: float, stream: int = 0) -> None:
     _check(lib().gpuann_chem_step(ctx, int(n_cells), T, p, Y, h, float(dt), stream or None), ctx)
+
+
+class gpuann_step_outputs(C.Structure):
+    _fields_ = [("rr", C.c_void_p), ("hrr", C.c_void_p), ("cp", C.c_void_p), ("rho", C.c_void_p), ("psi", C.c_void_p)]
+
+
+def gpuann_chem_step_ex(ctx: int, n_cells: int, T: int, p: int, Y: int, h: int, dt: float, stream: int = 0, *,
+                        rr: int = 0, hrr: int = 0, cp: int = 0, rho: int = 0, psi: int = 0) -> None:
+    """gpuann_chem_step plus the optional outputs (device addresses; 0 = not computed)."""
+    out = gpuann_step_outputs(rr or None, hrr or None, cp or None, rho or None, psi or None)
+    _check(lib().gpuann_chem_step_ex(ctx, int(n_cells), T, p, Y, h, float(dt), C.byref(out), stream or None), ctx)
 
 
 def gpuann_chem_step_host(ctx: int, n_cells: int, T: int, p: int, Y: int, h: int, dt: float) -> None:

@@ -422,6 +422,7 @@ int gpuann_load_thermo(gpuann_ctx *c, int n_species, const double *nasa_lo, cons
             h->hh[k][r][5] = s * a[4] / 5.0;
         }
         h->T_mid[k] = two ? T_mid[k] : 0.0;
+        h->inv_W[k] = 1.0 / W[k];
     }
     {
         TailArgs &ta = c->tail.args;  // the tail kernel takes the table by value (first kTailMaxNs species)
@@ -432,6 +433,7 @@ int gpuann_load_thermo(gpuann_ctx *c, int n_species, const double *nasa_lo, cons
             std::memcpy(ta.th.hh[k], h->hh[k], sizeof(ta.th.hh[k]));
             ta.th.T_mid[k] = h->T_mid[k];
         }
+        for (int k = 0; k < kTailMaxNs; ++k) ta.invW[k] = k < n_species ? (float)h->inv_W[k] : 0.f;
         std::memset(ta.hhf, 0, sizeof(ta.hhf));
         std::memset(ta.cpf, 0, sizeof(ta.cpf));
         for (int k = 0; k < kTailMaxNs && k < n_species; ++k) {
@@ -480,6 +482,7 @@ struct ChunkOut {
     float *T = nullptr, *Y = nullptr;  // update mode
     const float *h = nullptr;
     double dt = 0.0;
+    ExtraOut ex;              // gpuann_chem_step_ex
 };
 
 // the tensor path for the chunk [c0, c0+cn): z -> layers -> (raw output | update S4-S8)
@@ -495,7 +498,7 @@ int run_chunk_bf16(Ctx *c, int64_t n, int64_t c0, int64_t cn, const float *T, co
     const bool raw = out.o_raw != nullptr;
     for (int l = l0; l < c->L; ++l) {
         if (c->tail.on && l == c->L - 2) {
-            CU_TRY(c, launch_tail(c, n, c0, cn, out.T, out.Y, out.h, out.dt, out.o_raw, out.o_stride, use_idx, s), "tail kernel");
+            CU_TRY(c, launch_tail(c, n, c0, cn, out.T, p, out.Y, out.h, out.dt, out.o_raw, out.o_stride, use_idx, out.ex, s), "tail kernel");
             return GPUANN_OK;
         }
         const bool last = l == c->L - 1;
@@ -526,15 +529,30 @@ extern "C" {
 
 int gpuann_chem_step(gpuann_ctx *c, int64_t n, float *T, const float *p, float *Y, const float *h, double dt,
                      void *stream) {
+    return gpuann_chem_step_ex(c, n, T, p, Y, h, dt, nullptr, stream);
+}
+
+int gpuann_chem_step_ex(gpuann_ctx *c, int64_t n, float *T, const float *p, float *Y, const float *h, double dt,
+                        const gpuann_step_outputs *xo, void *stream) {
     if (!c) return fail(nullptr, GPUANN_ERR_INVALID_ARG, "gpuann_chem_step: ctx is NULL");
     int rc = check_step_args(c, "gpuann_chem_step", n, T, p, Y, h, dt, true);
     if (rc != GPUANN_OK) return rc;
     if (n == 0) return GPUANN_OK;
+    ExtraOut ex;
+    if (xo) {
+        ex.rr = xo->rr;
+        ex.hrr = xo->hrr;
+        ex.cp = xo->cp;
+        ex.rho = xo->rho;
+        ex.psi = xo->psi;
+    }
+    if (ex.any() && c->prm.precision == GPUANN_PRECISION_BF16 && !c->tail.on)
+        return fail(c, GPUANN_ERR_UNSUPPORTED, "gpuann_chem_step_ex: the extra outputs need the tail kernel (Ns <= 48, last hidden layer <= 416)");
     DeviceGuard g(c->device);
     cudaStream_t s = reinterpret_cast<cudaStream_t>(stream);
     c->last_stream = s;
     if (c->prm.precision == GPUANN_PRECISION_FP32) {
-        CU_TRY(c, launch_chem_fp32(c, n, T, p, Y, h, dt, nullptr, false, s), "fp32 kernel");
+        CU_TRY(c, launch_chem_fp32(c, n, T, p, Y, h, dt, nullptr, false, ex, s), "fp32 kernel");
         return GPUANN_OK;
     }
     const bool use_idx = c->prm.T_active > 0.0;
@@ -550,6 +568,7 @@ int gpuann_chem_step(gpuann_ctx *c, int64_t n, float *T, const float *p, float *
     out.Y = Y;
     out.h = h;
     out.dt = dt;
+    out.ex = ex;
     for (int64_t c0 = 0; c0 < n; c0 += c->chunk) {
         const int64_t cn = (n - c0) < c->chunk ? (n - c0) : c->chunk;
         rc = run_chunk_bf16(c, n, c0, cn, T, p, Y, use_idx, out, s);
@@ -569,7 +588,7 @@ int gpuann_debug_forward(gpuann_ctx *c, int64_t n, const float *T, const float *
     cudaStream_t s = reinterpret_cast<cudaStream_t>(stream);
     c->last_stream = s;
     if (c->prm.precision == GPUANN_PRECISION_FP32) {
-        CU_TRY(c, launch_chem_fp32(c, n, const_cast<float *>(T), p, const_cast<float *>(Y), nullptr, 1.0, o_raw, true, s),
+        CU_TRY(c, launch_chem_fp32(c, n, const_cast<float *>(T), p, const_cast<float *>(Y), nullptr, 1.0, o_raw, true, ExtraOut{}, s),
                "fp32 kernel");
         return GPUANN_OK;
     }

@@ -25,8 +25,15 @@ struct ThermoDev {
     double cp[kMaxSpecies][2][5];  // (Ru/W) a1..a5
     double hh[kMaxSpecies][2][6];  // (Ru/W) {a6, a1, a2/2, a3/3, a4/4, a5/5}
     double T_mid[kMaxSpecies];
+    double inv_W[kMaxSpecies];     // 1 / W_k [kmol/kg] (density, R_mix)
     int n_species;
     int two_ranges;
+};
+
+// optional outputs of gpuann_chem_step_ex (device pointers or nullptr)
+struct ExtraOut {
+    float *rr = nullptr, *hrr = nullptr, *cp = nullptr, *rho = nullptr, *psi = nullptr;
+    __host__ __device__ bool any() const { return rr || hrr || cp || rho || psi; }
 };
 
 // Everything the update S4-S7 needs besides the thermo table.
@@ -119,6 +126,11 @@ struct TailArgs {
     // FP32 copies of the one-range table for the FAST instance of the kernel (mixture coefficients accumulated in FP32)
     float hhf[kTailMaxNs][6];
     float cpf[kTailMaxNs][5];
+    // gpuann_chem_step_ex
+    const float *p;
+    ExtraOut ex;
+    float invW[kTailMaxNs];
+    float inv_dt;
 };
 struct TailNet {
     bool on = false;
@@ -233,7 +245,7 @@ struct LaunchScope {
 // ---------------------------------------------------------------- kernel launchers (defined in the .cu files)
 // k_fp32.cu
 cudaError_t launch_chem_fp32(Ctx *c, int64_t n, float *T, const float *p, float *Y, const float *h, double dt,
-                             float *o_raw, bool forward_only, cudaStream_t s);
+                             float *o_raw, bool forward_only, const ExtraOut &ex, cudaStream_t s);
 size_t fp32_smem_bytes(const Ctx *c, int *cells_per_block);
 
 // k_aux.cu
@@ -263,8 +275,8 @@ cudaError_t launch_fused_l1l2(Ctx *c, int64_t n, int64_t c0, int64_t cn, const f
 cudaError_t tail_setup(Ctx *c);
 bool tail_supported(int K3p, int H3p, int Ns);
 void tail_plan(int H3p, int *n0, int *n1);
-cudaError_t launch_tail(Ctx *c, int64_t n, int64_t c0, int64_t cn, float *T, float *Y, const float *h, double dt,
-                        float *o_raw, int64_t o_stride, bool use_idx, cudaStream_t s);
+cudaError_t launch_tail(Ctx *c, int64_t n, int64_t c0, int64_t cn, float *T, const float *p, float *Y, const float *h,
+                        double dt, float *o_raw, int64_t o_stride, bool use_idx, const ExtraOut &ex, cudaStream_t s);
 
 // encodes a 2-D BF16 row-major tensor map {inner = cols, outer = rows}, box {64, box_rows}, 128-byte swizzle
 bool encode_tmap_bf16(CUtensorMap *out, const void *base, uint64_t cols, uint64_t rows, uint64_t row_pitch_bytes,

@@ -33,7 +33,7 @@ __global__ void __launch_bounds__(kFp32Threads) k_chem_fp32(int64_t n, float *__
                                                             const float *__restrict__ b_g,
                                                             const ThermoDev *__restrict__ thermo,
                                                             Counters *__restrict__ counters, const Fp32Net net,
-                                                            const PreParams pre, const PostParams pp) {
+                                                            const PreParams pre, const PostParams pp, const ExtraOut ex) {
     extern __shared__ __align__(16) float smem[];
     constexpr int G = kFp32Threads / CB;
     float *act0 = smem;
@@ -128,6 +128,31 @@ __global__ void __launch_bounds__(kFp32Threads) k_chem_fp32(int64_t n, float *__
         bool conv;
         const double Tn = newton_T<kMaxSpecies>(Ys, Ns, (double)h[cell], (double)Tin, thermo, pp, &conv);
         if (!conv) nconv = 1;
+        if (ex.any()) {
+            // gpuann_chem_step_ex (include/gpuann.h; R19-R21), FP64, before the inputs are overwritten
+            double inv_w_in = 0.0, inv_w = 0.0, cpm = 0.0, q = 0.0;
+#pragma unroll 1
+            for (int k = 0; k < Ns; ++k) inv_w_in = fma(Yc[k], thermo->inv_W[k], inv_w_in);
+            const double rho_in = (double)p[cell] / (kRu * (double)Tin * inv_w_in);
+            const double rate = rho_in / dt;
+#pragma unroll 1
+            for (int k = 0; k < Ns; ++k) {
+                const int r = (thermo->two_ranges && !(Tn < thermo->T_mid[k])) ? 1 : 0;
+                const double *cpk = thermo->cp[k][r];
+                const double *hh = thermo->hh[k][r];
+                const double hk = hh[0] + Tn * (hh[1] + Tn * (hh[2] + Tn * (hh[3] + Tn * (hh[4] + Tn * hh[5]))));
+                const double rr = rate * (Ys[k] - (double)Y[(int64_t)k * n + cell]);
+                q = fma(-hk, rr, q);
+                cpm = fma(Ys[k], cpk[0] + Tn * (cpk[1] + Tn * (cpk[2] + Tn * (cpk[3] + Tn * cpk[4]))), cpm);
+                inv_w = fma(Ys[k], thermo->inv_W[k], inv_w);
+                if (ex.rr) ex.rr[(int64_t)k * n + cell] = (float)rr;
+            }
+            const double psi = 1.0 / (kRu * inv_w * Tn);
+            if (ex.hrr) ex.hrr[cell] = (float)q;
+            if (ex.cp) ex.cp[cell] = (float)cpm;
+            if (ex.rho) ex.rho[cell] = (float)((double)p[cell] * psi);
+            if (ex.psi) ex.psi[cell] = (float)psi;
+        }
 #pragma unroll 1
         for (int k = 0; k < Ns; ++k) Y[(int64_t)k * n + cell] = (float)Ys[k];
         T[cell] = (float)Tn;
@@ -160,7 +185,7 @@ size_t fp32_smem_bytes(const Ctx *c, int *cells_per_block) {
 }
 
 cudaError_t launch_chem_fp32(Ctx *c, int64_t n, float *T, const float *p, float *Y, const float *h, double dt,
-                             float *o_raw, bool forward_only, cudaStream_t s) {
+                             float *o_raw, bool forward_only, const ExtraOut &ex, cudaStream_t s) {
     if (n <= 0) return cudaSuccess;
     int cb = 0;
     const size_t smem = fp32_smem_bytes(c, &cb);
@@ -190,7 +215,7 @@ cudaError_t launch_chem_fp32(Ctx *c, int64_t n, float *T, const float *p, float 
         if (e == cudaSuccess)                                                                                        \
             k_chem_fp32<CB><<<blocks, kFp32Threads, smem, s>>>(n, T, p, Y, h, dt, o_raw, forward_only ? 1 : 0, Tact, \
                                                                c->w32, c->b32, c->thermo_dev, c->counters, net,     \
-                                                               c->pre, c->post);                                     \
+                                                               c->pre, c->post, ex);                                 \
     } while (0)
     if (cb == 32) GPUANN_LAUNCH_FP32(32);
     else if (cb == 16) GPUANN_LAUNCH_FP32(16);

@@ -353,13 +353,16 @@ k_tail(const __grid_constant__ CUtensorMap tmapA /* row-major [rows][K3p] or blo
             const uint32_t ob = (uint32_t)it & 1u, oph = ((uint32_t)it >> 1) & 1u;
             // state loads first: their latency hides behind the wait for o
             float Yv[NSP];
-            float Tin = 300.f, hin = 0.f;
+            float Tin = 300.f, hin = 0.f, pin = 101325.f;
+            const bool ex_any = ta.ex.any();  // gpuann_chem_step_ex (include/gpuann.h; R19-R21)
+            float inv_w_in = 0.f, inv_w_new = 0.f;
             if (!fwd_only) {
 #pragma unroll
                 for (int k = 0; k < NSP; ++k) Yv[k] = (valid && k < Ns) ? ta.Y[(int64_t)k * ta.n + g] : 0.f;
                 if (valid) {
                     Tin = ta.T[g];
                     hin = ta.h[g];
+                    if (ex_any) pin = ta.p[g];
                 }
             }
             ptx::mbar_wait(&bars[tOFull + ob], oph);
@@ -407,6 +410,10 @@ k_tail(const __grid_constant__ CUtensorMap tmapA /* row-major [rows][K3p] or blo
                         ys = update_species_f32(yc, dy, ta);
                     }
                     Yv[k] = ys;
+                    if (ex_any) {
+                        inv_w_in = fmaf(yc, ta.invW[k], inv_w_in);
+                        inv_w_new = fmaf(ys, ta.invW[k], inv_w_new);
+                    }
                     if (FAST) {
                         Sf += ys;
 #pragma unroll
@@ -436,9 +443,11 @@ k_tail(const __grid_constant__ CUtensorMap tmapA /* row-major [rows][K3p] or blo
                 for (int m = 0; m < 5; ++m) Cc[m] = 0.0;
 #pragma unroll 1
                 for (int k = 0; k < Ns; ++k) S += (double)fmaxf(valid ? ta.Y[(int64_t)k * ta.n + g] : 0.f, 0.f);
+                inv_w_new = 0.f;
 #pragma unroll
                 for (int k = 0; k < NSP; ++k) {
                     Yv[k] = (valid && k < Ns) ? fmaxf(ta.Y[(int64_t)k * ta.n + g], 0.f) : 0.f;
+                    inv_w_new = fmaf(Yv[k], ta.invW[k], inv_w_new);
                     const double yd = (double)Yv[k];
 #pragma unroll
                     for (int m = 0; m < 6; ++m) Ch[m] = fma(yd, ta.th.hh[k][0][m], Ch[m]);
@@ -501,6 +510,36 @@ k_tail(const __grid_constant__ CUtensorMap tmapA /* row-major [rows][K3p] or blo
                     conv = true;
                     break;
                 }
+            }
+            // gpuann_chem_step_ex: the inputs are read once more (cache hits) before they are overwritten
+            if (ex_any && valid) {
+                const float Tnf = (float)Tn;
+                const float rate = pin / (8314.46261815324f * Tin * inv_w_in) * ta.inv_dt;  // rho of the input state / dt
+                float q = 0.f, cpm = 0.f;
+#pragma unroll
+                for (int k = 0; k < NSP; ++k) {
+                    if (k < Ns) {
+                        const float ynew = FAST ? Yv[k] * rSf : (float)((double)Yv[k] * rS);
+                        const float rr = rate * (ynew - ta.Y[(int64_t)k * ta.n + g]);
+                        float hk;
+                        if (FAST || !ta.two_ranges) {
+                            const float *hh = ta.hhf[k];
+                            hk = hh[0] + Tnf * (hh[1] + Tnf * (hh[2] + Tnf * (hh[3] + Tnf * (hh[4] + Tnf * hh[5]))));
+                        } else {
+                            const int rg = !(Tn < ta.th.T_mid[k]) ? 1 : 0;
+                            hk = (float)horner6(ta.th.hh[k][rg], Tn);
+                            cpm = fmaf(ynew, (float)horner5(ta.th.cp[k][rg], Tn), cpm);
+                        }
+                        q = fmaf(-hk, rr, q);
+                        if (ta.ex.rr) ta.ex.rr[(int64_t)k * ta.n + g] = rr;
+                    }
+                }
+                if (FAST || !ta.two_ranges) cpm = (float)horner5(Cc, Tn);  // the mixture coefficients are already those of Y_new
+                const float psi = 1.f / (8314.46261815324f * (inv_w_new * rSf) * Tnf);
+                if (ta.ex.hrr) ta.ex.hrr[g] = q;
+                if (ta.ex.cp) ta.ex.cp[g] = cpm;
+                if (ta.ex.rho) ta.ex.rho[g] = pin * psi;
+                if (ta.ex.psi) ta.ex.psi[g] = psi;
             }
             // S8: store in place (skipped / out-of-range cells are never touched)
             if (valid) {
@@ -569,8 +608,8 @@ void tail_plan(int H3p, int *n0, int *n1) {
     *n1 = b;
 }
 
-cudaError_t launch_tail(Ctx *c, int64_t n, int64_t c0, int64_t cn, float *T, float *Y, const float *h, double dt,
-                        float *o_raw, int64_t o_stride, bool use_idx, cudaStream_t s) {
+cudaError_t launch_tail(Ctx *c, int64_t n, int64_t c0, int64_t cn, float *T, const float *p, float *Y, const float *h,
+                        double dt, float *o_raw, int64_t o_stride, bool use_idx, const ExtraOut &ex, cudaStream_t s) {
     if (cn <= 0) return cudaSuccess;
     TailNet &tn = c->tail;
     TailArgs &ta = tn.args;  // the constant part (thermo, net parameters) was filled at load time
@@ -583,6 +622,9 @@ cudaError_t launch_tail(Ctx *c, int64_t n, int64_t c0, int64_t cn, float *T, flo
     ta.T = T;
     ta.Y = Y;
     ta.h = h;
+    ta.p = p;
+    ta.ex = ex;
+    ta.inv_dt = (float)(1.0 / dt);
     ta.o_raw = o_raw;
     ta.o_stride = o_stride;
     ta.counters = c->counters;

@@ -209,3 +209,74 @@ def subset(pr: Prepared, g: GpuResult, idx):
     sub = GpuResult(g.T_new[idx], np.ascontiguousarray(g.Y_new[:, idx]),
                     None if g.o_raw is None else np.ascontiguousarray(g.o_raw[:, idx]), g.stats)
     return ref, sub
+
+
+# ------------------------------------------------------------------ gpuann_chem_step_ex (O8 / O9; R19-R22)
+def run_gpu_ex(ctx: int, pr: Prepared, which=("rr", "hrr", "cp", "rho", "psi")):
+    """One gpuann_chem_step_ex on the prepared state.  Returns (GpuResult, dict of the requested outputs); outputs are
+    pre-filled with NaN so that an entry the library did not write is visible."""
+    import torch
+    st = pr.prob.state
+    n = int(st.T.shape[0])
+    Ns = pr.prob.cfg.n_species
+    dev = torch.device("cuda:0")
+    dT, dp, dY, dh = (torch.from_numpy(np.ascontiguousarray(a)).to(dev) for a in (st.T, st.p, st.Y, pr.h))
+    bufs = {k: torch.full((Ns, n) if k == "rr" else (n,), float("nan"), dtype=torch.float32, device=dev) for k in which}
+    stream = torch.cuda.current_stream().cuda_stream
+    B.gpuann_reset_stats(ctx)
+    B.gpuann_chem_step_ex(ctx, n, dT.data_ptr(), dp.data_ptr(), dY.data_ptr(), dh.data_ptr(), pr.prob.cfg.dt, stream,
+                          **{k: v.data_ptr() for k, v in bufs.items()})
+    torch.cuda.synchronize()
+    return (GpuResult(dT.cpu().numpy(), dY.cpu().numpy(), None, B.gpuann_get_stats(ctx)),
+            {k: v.cpu().numpy().astype(np.float64) for k, v in bufs.items()})
+
+
+def check_ex(pr: Prepared, ref, ex: dict, bf16: bool, lam: float = 0.1):
+    """Element-wise gates on the extra outputs, derived from the gates on Y_new and T_new (R22):
+    RR_k = rho (Y_new,k - Y_k)/dt inherits tol(Y_new,k) rho/dt (+ FP32 output rounding); HRR = -sum h_k RR_k inherits
+    sum_k |h_k| tol(RR_k); cp, rho, psi move with T_new (0.5 K / 1e-3 K) and Y_new (2e-3 / 1e-5)."""
+    st, th, cfg = pr.prob.state, pr.prob.thermo, pr.prob.cfg
+    der = oracle.Oracle(pr.model).derived(st.T, st.p, st.Y, cfg.dt, ref)
+    act = ref.flags != 4
+    Yr = ref.Y_new
+    if bf16:
+        with np.errstate(divide="ignore"):
+            sens = np.maximum(1.0, 0.19 / np.power(np.abs(Yr), lam)) if lam > 0 else np.ones_like(Yr)
+        sens = np.where(np.isfinite(sens), sens, 1.0)
+        tolY = 2e-3 * sens * np.abs(Yr) + 1e-10
+        rel_T = 0.5 / ref.T_new + 2e-3
+    else:
+        tolY = 1e-5 * np.abs(Yr) + 1e-10
+        rel_T = 1e-3 / ref.T_new + 1e-5
+    Yc = np.maximum(st.Y.astype(np.float64), 0.0)
+    rho_in = st.p.astype(np.float64) / (8314.46261815324 * st.T.astype(np.float64) * (Yc / th.W[:, None]).sum(axis=0))
+    tolRR = rho_in / cfg.dt * (tolY + 2e-7 * np.abs(st.Y.astype(np.float64))) + 1e-5 * np.abs(der.rr)
+    out = {}
+    if "rr" in ex:
+        err = np.abs(ex["rr"] - der.rr)[:, act]
+        assert np.isfinite(ex["rr"][:, act]).all()
+        out["rr"] = (err / tolRR[:, act]).max()
+        assert out["rr"] <= 1.0, f"RR: max err/tol = {out['rr']:.3f}"
+        assert np.isnan(ex["rr"][:, ~act]).all(), "RR of a skipped cell was written"
+    if "hrr" in ex:
+        hk = np.empty_like(Yr)
+        for k in range(Yr.shape[0]):
+            lo = th.nasa_lo[k]
+            hi = lo if th.nasa_hi is None else th.nasa_hi[k]
+            a = np.where((ref.T_new < (th.T_mid[k] if th.T_mid is not None else np.inf))[:, None], lo[None, :], hi[None, :])
+            T = ref.T_new
+            hk[k] = 8314.46261815324 / th.W[k] * (a[:, 0] * T + a[:, 1] * T ** 2 / 2 + a[:, 2] * T ** 3 / 3
+                                                  + a[:, 3] * T ** 4 / 4 + a[:, 4] * T ** 5 / 5 + a[:, 5])
+        # h_k itself moves with T_new: |dh_k| <= cp_k dT, folded in through rel_T on the sum of |h_k RR_k|
+        tolH = (np.abs(hk) * tolRR).sum(axis=0) + rel_T * (np.abs(hk) * np.abs(der.rr)).sum(axis=0)
+        err = np.abs(ex["hrr"] - der.hrr)[act]
+        out["hrr"] = (err / tolH[act]).max()
+        assert out["hrr"] <= 1.0, f"HRR: max err/tol = {out['hrr']:.3f}"
+        assert np.isnan(ex["hrr"][~act]).all()
+    for name, want in (("cp", der.cp), ("rho", der.rho_new), ("psi", der.psi)):
+        if name in ex:
+            err = np.abs(ex[name] - want)[act] / (rel_T[act] * np.abs(want[act]))
+            out[name] = err.max()
+            assert out[name] <= 1.0, f"{name}: max err/tol = {out[name]:.3f}"
+            assert np.isnan(ex[name][~act]).all()
+    return out

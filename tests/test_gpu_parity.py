@@ -323,3 +323,66 @@ def test_host_variant_equals_device_variant(n, chunk):
         assert np.array_equal(ph.numpy(), st.p) and np.array_equal(hh.numpy(), pr.h)  # read-only inputs untouched
     finally:
         B.gpuann_destroy(ctx)
+
+
+# ------------------------------------------------------------------ gpuann_chem_step_ex: RR, HRR, cp, rho, psi
+def test_ex_outputs_fp32_c0():
+    pr = G.prepare(I.get_config("c0"))
+    ctx = G.make_ctx(pr)
+    try:
+        g, ex = G.run_gpu_ex(ctx, pr)
+        ref = G.run_oracle(pr)
+        G.check_fp32(g, ref)                       # the step itself is unchanged by the extra outputs
+        w = G.check_ex(pr, ref, ex, bf16=False)
+        print(f"c0 ex: {w}")
+    finally:
+        B.gpuann_destroy(ctx)
+
+
+@pytest.mark.parametrize("name,n", [("c2", 128 * 11 + 53), ("c3", 128 * 5 + 1), ("c1", 4099)])
+def test_ex_outputs_bf16(name, n):
+    pr = G.prepare(I.get_config(name), n=n, seed=77)
+    ctx = G.make_ctx(pr)
+    try:
+        g, ex = G.run_gpu_ex(ctx, pr)
+        ref = G.run_oracle(pr)
+        G.check_T_bf16(g, ref)
+        G.check_Y_bf16(g, ref)
+        w = G.check_ex(pr, ref, ex, bf16=True)
+        # asking for the extra outputs must not change the step: bit-identical T, Y with and without them
+        g0 = G.run_gpu(ctx, pr, want_raw=False)
+        assert np.array_equal(g0.T_new, g.T_new) and np.array_equal(g0.Y_new, g.Y_new)
+        print(f"{name} ex: {w}")
+    finally:
+        B.gpuann_destroy(ctx)
+
+
+def test_ex_outputs_subset_and_skipped_cells_c4():
+    """Only some outputs requested; cells below T_active are not written (NaN pre-fill survives)."""
+    pr = G.prepare(I.get_config("c4"), n=128 * 9 + 17, seed=5)
+    ctx = G.make_ctx(pr)
+    try:
+        g, ex = G.run_gpu_ex(ctx, pr, which=("hrr", "rho"))
+        ref = G.run_oracle(pr)
+        act = ref.flags != 4
+        assert 0 < act.sum() < act.size
+        G.check_T_bf16(g, ref, act)
+        w = G.check_ex(pr, ref, ex, bf16=True)
+        print(f"c4 ex: {w}")
+    finally:
+        B.gpuann_destroy(ctx)
+
+
+def test_ex_outputs_two_range_thermo():
+    """The generic (non-FAST) instance of the tail kernel: two NASA-7 ranges, T_mid inside the batch's T range."""
+    pr = G.prepare(I.get_config("c2"), n=128 * 3 + 9, seed=9,
+                   mutate=lambda prob: _continuous_two_range(prob, np.random.default_rng(5)))
+    ctx = G.make_ctx(pr)
+    try:
+        g, ex = G.run_gpu_ex(ctx, pr)
+        ref = G.run_oracle(pr)
+        G.check_T_bf16(g, ref)
+        w = G.check_ex(pr, ref, ex, bf16=True)
+        print(f"two-range ex: {w}")
+    finally:
+        B.gpuann_destroy(ctx)

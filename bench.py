@@ -202,7 +202,7 @@ def run_reference(args, rank: int, world: int):
 
 def workload_name(cfg, n):
     return (f"configs[{cfg.index}]: {n} cells, Ns={cfg.n_species}, MLP {'-'.join(str(s) for s in cfg.sizes)} GELU, "
-            f"{'BF16 tcgen05' if cfg.precision == 1 else 'FP32'}, dt={cfg.dt:g}s")
+            f"{ {0: 'FP32', 1: 'BF16 tcgen05', 2: 'FP16 tcgen05'}[cfg.precision] }, dt={cfg.dt:g}s")
 
 
 # ------------------------------------------------------------------ our arm
@@ -426,7 +426,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_total / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "bf16" if cfg.precision == 1 else "f32",
+            "scaling": "weak", "vs_baseline": None, "dtype": {0: "f32", 1: "bf16", 2: "f16"}[cfg.precision],
             "data": "synthetic",
             "config": {"workload": workload_name(cfg, n), "cells_per_gpu": n, "variant": variant + ("+ex(rr,hrr,cp,rho,psi)" if args.ex else ""),
                        "l2": "state (184 B/cell x n) larger than L2 and restored from a pristine copy between steps",

@@ -60,6 +60,11 @@ typedef enum {
 
 #define GPUANN_PRECISION_FP32 0 /* CUDA-core FP32 MLP, exact-erf GELU (configs[0]) */
 #define GPUANN_PRECISION_BF16 1 /* tcgen05 BF16 x BF16 -> FP32 MLP, activations rounded to BF16 (configs[1..4]) */
+#define GPUANN_PRECISION_FP16 2 /* the same kernels with FP16 weights and activations, FP32 accumulate: the half precision
+                                   the paper infers in.  Weights are rounded to FP16
+                                   (values that are FP16-representable are used exactly; |w| must stay below 65504).
+                                   Only nets that run the fused + tail kernels (4 weight matrices, Ns <= 48,
+                                   last hidden layer <= 416, first hidden layer >= 128): UNSUPPORTED otherwise */
 
 /* Parameters of a context.  gpuann_default_params fills the defaults; passing NULL to gpuann_create
  * is the same as passing the defaults. */

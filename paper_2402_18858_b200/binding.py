@@ -22,6 +22,7 @@ GPUANN_ERR_ALLOC = 4
 GPUANN_ERR_CUDA = 5
 GPUANN_PRECISION_FP32 = 0
 GPUANN_PRECISION_BF16 = 1
+GPUANN_PRECISION_FP16 = 2
 
 # every symbol include/gpuann.h declares (tests check that the library exports all of them)
 SYMBOLS = [

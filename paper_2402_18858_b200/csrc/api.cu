@@ -5,6 +5,7 @@
 #include <cstring>
 #include <new>
 
+#include <cuda_fp16.h>
 #include "common.cuh"
 
 using namespace gpuann;
@@ -57,6 +58,19 @@ inline uint16_t f32_to_bf16_rne(float f) {
     return (uint16_t)(u >> 16);
 }
 
+// FP32 -> FP16 bits, round to nearest even (overflow -> inf, subnormals kept)
+inline uint16_t f32_to_f16_rne(float f) {
+    const __half h = __float2half_rn(f);
+    uint16_t u;
+    std::memcpy(&u, &h, 2);
+    return u;
+}
+inline float f16_bits_to_f32(uint16_t u) {
+    __half h;
+    std::memcpy(&h, &u, 2);
+    return __half2float(h);
+}
+
 void free_net(Ctx *c) {
     cudaFree(c->w32);
     cudaFree(c->b32);
@@ -105,8 +119,8 @@ int gpuann_create(const gpuann_params *params, gpuann_ctx **out) {
     gpuann_params prm;
     gpuann_default_params(&prm);
     if (params) prm = *params;
-    if (prm.precision != GPUANN_PRECISION_FP32 && prm.precision != GPUANN_PRECISION_BF16)
-        return fail(nullptr, GPUANN_ERR_INVALID_ARG, "gpuann_create: precision must be 0 (FP32) or 1 (BF16)");
+    if (prm.precision != GPUANN_PRECISION_FP32 && prm.precision != GPUANN_PRECISION_BF16 && prm.precision != GPUANN_PRECISION_FP16)
+        return fail(nullptr, GPUANN_ERR_INVALID_ARG, "gpuann_create: precision must be 0 (FP32), 1 (BF16) or 2 (FP16)");
     if (prm.newton_max_iter < 0 || !(prm.newton_tol > 0.0) || !(prm.T_min > 0.0) || !(prm.T_max > prm.T_min) ||
         !std::isfinite(prm.T_active))
         return fail(nullptr, GPUANN_ERR_INVALID_ARG,
@@ -145,9 +159,9 @@ int gpuann_create(const gpuann_params *params, gpuann_ctx **out) {
     if (e == cudaSuccess) e = cudaMemset(c->n_active_dev, 0, sizeof(int32_t));
     if (e == cudaSuccess) e = cudaMalloc(&c->thermo_dev, sizeof(ThermoDev));
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->own_stream, cudaStreamNonBlocking);
-    if (e == cudaSuccess && prm.precision == GPUANN_PRECISION_BF16) e = gemm_setup(c);
-    if (e == cudaSuccess && prm.precision == GPUANN_PRECISION_BF16) e = fused_setup(c);
-    if (e == cudaSuccess && prm.precision == GPUANN_PRECISION_BF16) e = tail_setup(c);
+    if (e == cudaSuccess && prm.precision != GPUANN_PRECISION_FP32) e = gemm_setup(c);
+    if (e == cudaSuccess && prm.precision != GPUANN_PRECISION_FP32) e = fused_setup(c);
+    if (e == cudaSuccess && prm.precision != GPUANN_PRECISION_FP32) e = tail_setup(c);
     if (e != cudaSuccess) {
         int rc = fail_cuda(nullptr, e, "gpuann_create");
         gpuann_destroy(c);
@@ -258,11 +272,15 @@ int gpuann_load_net(gpuann_ctx *c, int n_species, int n_layers, const int *sizes
     // ---- BF16 tensor path: pad, round (RNE), upload, encode the tensor maps
     // variant: "bf16-fused" (S1 + S2 + layers 1-2 in one kernel, k_fused.cu) when the shapes allow it, else
     // "bf16-layerwise"
+    const bool f16 = c->prm.precision == GPUANN_PRECISION_FP16;
+    auto to_half = [f16](float v) { return f16 ? f32_to_f16_rne(v) : f32_to_bf16_rne(v); };
     const bool fused = n_layers >= 3 && fused_supported(sizes[0], sizes[1], pad16(sizes[2]));
     // "+tail": the last two layers and the update S4-S8 in one kernel (k_tail.cu); needs a layer in front of them
     // (the fused kernel or a GEMM) that leaves their input in an activation buffer
     const bool tail = n_layers >= (fused ? 4 : 2) &&
                       tail_supported(pad16(sizes[n_layers - 2]), pad16(sizes[n_layers - 1]), n_species);
+    if (f16 && !(fused && tail && n_layers == 4))
+        return fail(c, GPUANN_ERR_UNSUPPORTED, "gpuann_load_net: GPUANN_PRECISION_FP16 needs a net the fused + tail kernels run (4 weight matrices)");
     int64_t chunk = c->prm.chunk_cells > 0 ? c->prm.chunk_cells : (int64_t)c->sm_count * 128 * (fused ? 56 : 1);
     chunk = (chunk + 127) / 128 * 128;
     c->chunk = chunk;
@@ -285,7 +303,7 @@ int gpuann_load_net(gpuann_ctx *c, int n_species, int n_layers, const int *sizes
         // every hidden activation is stored as 2 GELU(.) (ptx::gelu2_pack): its consumer W_l, l >= 1, carries the 1/2
         const float wscale = l >= 1 ? 0.5f : 1.f;
         for (int j = 0; j < ly.N; ++j) {
-            for (int i = 0; i < ly.K; ++i) hw[(size_t)j * ly.Kp + i] = f32_to_bf16_rne(wscale * weights[l][(size_t)j * ly.K + i]);
+            for (int i = 0; i < ly.K; ++i) hw[(size_t)j * ly.Kp + i] = to_half(wscale * weights[l][(size_t)j * ly.K + i]);
             hb[j] = biases[l][j];
         }
         CU_TRY(c, cudaMalloc(&ly.W, hw.size() * sizeof(uint16_t)), "cudaMalloc(W bf16)");
@@ -305,14 +323,18 @@ int gpuann_load_net(gpuann_ctx *c, int n_species, int n_layers, const int *sizes
         const int H1p = (H1 + 63) / 64 * 64;  // rows up to the next multiple of 64 stay zero: h1 = 0 there (k_fused.cu)
         std::vector<uint16_t> w1((size_t)H1p * 64, 0);
         for (int j = 0; j < H1; ++j) {
-            for (int i = 0; i < D; ++i) w1[(size_t)j * 64 + i] = f32_to_bf16_rne(weights[0][(size_t)j * D + i]);
+            for (int i = 0; i < D; ++i) w1[(size_t)j * 64 + i] = to_half(weights[0][(size_t)j * D + i]);
             const float b = biases[0][j];
-            const uint16_t hi = f32_to_bf16_rne(b);
-            uint32_t hbits = (uint32_t)hi << 16;
+            const uint16_t hi = to_half(b);
             float hf;
-            std::memcpy(&hf, &hbits, 4);
+            if (f16) {
+                hf = f16_bits_to_f32(hi);
+            } else {
+                uint32_t hbits = (uint32_t)hi << 16;
+                std::memcpy(&hf, &hbits, 4);
+            }
             w1[(size_t)j * 64 + D] = hi;
-            w1[(size_t)j * 64 + D + 1] = f32_to_bf16_rne(b - hf);
+            w1[(size_t)j * 64 + D + 1] = to_half(b - hf);
         }
         CU_TRY(c, cudaMalloc(&fn.W1p, w1.size() * sizeof(uint16_t)), "cudaMalloc(W1 padded)");
         CU_TRY(c, cudaMemcpy(fn.W1p, w1.data(), w1.size() * sizeof(uint16_t), cudaMemcpyHostToDevice), "cudaMemcpy(W1 padded)");
@@ -381,7 +403,8 @@ int gpuann_load_net(gpuann_ctx *c, int n_species, int n_layers, const int *sizes
         tn.on = true;
     }
     c->issued_mac_per_cell = mac;
-    c->variant = fused ? (tail ? "bf16-fused+tail" : "bf16-fused") : (tail ? "bf16-layerwise+tail" : "bf16-layerwise");
+    c->variant = f16 ? "fp16-fused+tail"
+                     : (fused ? (tail ? "bf16-fused+tail" : "bf16-fused") : (tail ? "bf16-layerwise+tail" : "bf16-layerwise"));
     c->net_loaded = true;
     return GPUANN_OK;
 }
@@ -546,7 +569,7 @@ int gpuann_chem_step_ex(gpuann_ctx *c, int64_t n, float *T, const float *p, floa
         ex.rho = xo->rho;
         ex.psi = xo->psi;
     }
-    if (ex.any() && c->prm.precision == GPUANN_PRECISION_BF16 && !c->tail.on)
+    if (ex.any() && c->prm.precision != GPUANN_PRECISION_FP32 && !c->tail.on)
         return fail(c, GPUANN_ERR_UNSUPPORTED, "gpuann_chem_step_ex: the extra outputs need the tail kernel (Ns <= 48, last hidden layer <= 416)");
     DeviceGuard g(c->device);
     cudaStream_t s = reinterpret_cast<cudaStream_t>(stream);
@@ -621,7 +644,7 @@ int gpuann_chem_step_host(gpuann_ctx *c, int64_t n, float *T, const float *p, fl
     float *dT = c->stage, *dp = dT + n, *dh = dp + n, *dY = dh + n;
     cudaStream_t s = c->own_stream;
     const size_t fb = (size_t)n * sizeof(float);
-    const bool pipelined = c->prm.precision == GPUANN_PRECISION_BF16 && !(c->prm.T_active > 0.0) && n >= 4 * 128 * (int64_t)c->sm_count;
+    const bool pipelined = c->prm.precision != GPUANN_PRECISION_FP32 && !(c->prm.T_active > 0.0) && n >= 4 * 128 * (int64_t)c->sm_count;
     if (!pipelined) {
         CU_TRY(c, cudaMemcpyAsync(dT, T, fb, cudaMemcpyHostToDevice, s), "H2D T");
         CU_TRY(c, cudaMemcpyAsync(dp, p, fb, cudaMemcpyHostToDevice, s), "H2D p");

@@ -113,6 +113,7 @@ struct TailArgs {
     int64_t o_stride;
     int Ns, Np;    // species, padded to 16
     int K3p, H3p, n0, n1;
+    int f16;        // 1: FP16 operands (GPUANN_PRECISION_FP16), 0: BF16
     int a_blocked;  // 1: the input activation is in the blocked layout the fused kernel writes (see FusedNet)
     const float *bias3;
     int newton_max_iter, inv_lambda_int, lambda_zero, two_ranges;

@@ -93,6 +93,7 @@ struct FusedArgs {
     const float *bias2;      // [H2p]
     __nv_bfloat16 *h2;       // [rows][H2p] row-major, or blocked [tile][H2p / 8][128][8] (common.cuh, FusedNet)
     int h2_blocked;
+    int f16;                 // 1: FP16 operands (GPUANN_PRECISION_FP16), 0: BF16
     PreParams pre;
 };
 
@@ -107,6 +108,8 @@ struct Ring {
     }
 };
 
+// F16: FP16 operands (GPUANN_PRECISION_FP16) instead of BF16 -- a template parameter so that the BF16 instance pays nothing
+template <bool F16>
 __global__ void __launch_bounds__(kFusedThreads, 1)
 k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__ CUtensorMap tmapW2a,
              const __grid_constant__ CUtensorMap tmapW2b, const __grid_constant__ FusedArgs fa) {
@@ -118,6 +121,7 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
     const uint32_t sbase = ptx::smem_u32(smem);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    constexpr bool f16 = F16;
 
     int64_t rows = fa.rows;
     if (fa.n_active) {
@@ -207,8 +211,8 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
     } else if (warp == kWarpMma2) {
         // ================================================================ layer-2 MMA issuer (leader; whole warp, uniform)
         if (leader && total_steps > 0) {
-            const uint32_t idesc_n0 = ptx::umma_idesc_bf16_f32(2 * kFM, (uint32_t)fa.n0);
-            const uint32_t idesc_n1 = ptx::umma_idesc_bf16_f32(2 * kFM, (uint32_t)(fa.n1 > 0 ? fa.n1 : 16));
+            const uint32_t idesc_n0 = ptx::umma_idesc_bf16_f32(2 * kFM, (uint32_t)fa.n0, F16);
+            const uint32_t idesc_n1 = ptx::umma_idesc_bf16_f32(2 * kFM, (uint32_t)(fa.n1 > 0 ? fa.n1 : 16), F16);
             const uint64_t b1_off = (uint64_t)((uint32_t)(fa.n0 / 2) * 128u >> 4);
             Ring w2;
             uint32_t slot = 0, a_ph = 0 /* bit s: parity of slot s's next "converted" phase */, acc_ph = 0;
@@ -249,7 +253,7 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
     } else if (warp == kWarpMma1) {
         // ================================================================ layer-1 MMA issuer (leader; whole warp, uniform)
         if (leader && total_steps > 0) {
-            const uint32_t idesc_l1 = ptx::umma_idesc_bf16_f32(2 * kFM, kSub);
+            const uint32_t idesc_l1 = ptx::umma_idesc_bf16_f32(2 * kFM, kSub, F16);
             Ring w1;
             int j1 = 0, pass1 = 0, it1 = 0;
             uint32_t slot1 = 0, s_ph = 0x7u;  // first use of every slot: nothing to wait for
@@ -353,8 +357,8 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
                 for (int q = 0; q < 4; ++q) {
                     const int rr = 4 * lane + q;
                     ptx::st_shared_v4(z_addr + (uint32_t)rr * 128u + (uint32_t)((u ^ (rr & 7)) << 4),
-                                      ptx::pack_bf16x2(x[q][0], x[q][1]), ptx::pack_bf16x2(x[q][2], x[q][3]),
-                                      ptx::pack_bf16x2(x[q][4], x[q][5]), ptx::pack_bf16x2(x[q][6], x[q][7]));
+                                      ptx::pack_half2(x[q][0], x[q][1], f16), ptx::pack_half2(x[q][2], x[q][3], f16),
+                                      ptx::pack_half2(x[q][4], x[q][5], f16), ptx::pack_half2(x[q][6], x[q][7], f16));
                 }
             }
             ptx::fence_proxy_async_smem();
@@ -418,8 +422,8 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
 #pragma unroll
                 for (int jj = 0; jj < 8; ++jj) {
                     const float4 bb = (full || jj < 4) ? b4[jj] : make_float4(0.f, 0.f, 0.f, 0.f);
-                    o[2 * jj] = ptx::gelu2_pack(__uint_as_float(v[4 * jj]) + bb.x, __uint_as_float(v[4 * jj + 1]) + bb.y);
-                    o[2 * jj + 1] = ptx::gelu2_pack(__uint_as_float(v[4 * jj + 2]) + bb.z, __uint_as_float(v[4 * jj + 3]) + bb.w);
+                    o[2 * jj] = ptx::gelu2_pack(__uint_as_float(v[4 * jj]) + bb.x, __uint_as_float(v[4 * jj + 1]) + bb.y, f16);
+                    o[2 * jj + 1] = ptx::gelu2_pack(__uint_as_float(v[4 * jj + 2]) + bb.z, __uint_as_float(v[4 * jj + 3]) + bb.w, f16);
                 }
                 if (fa.h2_blocked) {
                     // lane = row, one 16-byte piece per instruction: 512 contiguous bytes per warp instruction.  Rows past
@@ -458,7 +462,7 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
             ptx::tmem_ld_wait();
             uint32_t o[16];
 #pragma unroll
-            for (int jj = 0; jj < 16; ++jj) o[jj] = ptx::gelu2_pack(__uint_as_float(v[2 * jj]), __uint_as_float(v[2 * jj + 1]));
+            for (int jj = 0; jj < 16; ++jj) o[jj] = ptx::gelu2_pack(__uint_as_float(v[2 * jj]), __uint_as_float(v[2 * jj + 1]), f16);
             ptx::tmem_st16(slot_addr, o);
             ptx::tmem_st_wait();
             ptx::tc_fence_before_sync();
@@ -485,7 +489,9 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
 // ---------------------------------------------------------------- host side
 cudaError_t fused_setup(Ctx *c) {
     (void)c;
-    return cudaFuncSetAttribute(k_fused_l1l2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFusedSmem);
+    cudaError_t e = cudaFuncSetAttribute(k_fused_l1l2<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFusedSmem);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_fused_l1l2<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFusedSmem);
 }
 
 // H1 need not be a multiple of 64: W1 gets zero rows up to the next multiple (h1 = 2 GELU(0) = 0 there) and TMA zero-fills
@@ -532,6 +538,7 @@ cudaError_t launch_fused_l1l2(Ctx *c, int64_t n, int64_t c0, int64_t cn, const f
     fa.bias2 = c->lay[1].bias;
     fa.h2 = c->act[0];
     fa.h2_blocked = fn.h2_blocked ? 1 : 0;
+    fa.f16 = c->prm.precision == GPUANN_PRECISION_FP16 ? 1 : 0;
     fa.pre = c->pre;
     const int64_t tiles = (cn + kFM - 1) / kFM;
     int grid = (int)(tiles < c->sm_count ? tiles : c->sm_count);
@@ -549,7 +556,8 @@ cudaError_t launch_fused_l1l2(Ctx *c, int64_t n, int64_t c0, int64_t cn, const f
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, k_fused_l1l2, fn.tmapW1, fn.tmapW2a, fn.tmapW2b, fa);
+    if (fa.f16) return cudaLaunchKernelEx(&cfg, k_fused_l1l2<true>, fn.tmapW1, fn.tmapW2a, fn.tmapW2b, fa);
+    return cudaLaunchKernelEx(&cfg, k_fused_l1l2<false>, fn.tmapW1, fn.tmapW2a, fn.tmapW2b, fa);
 }
 
 }  // namespace gpuann

@@ -204,8 +204,8 @@ k_tail(const __grid_constant__ CUtensorMap tmapA /* row-major [rows][K3p] or blo
     } else if (warp == 1) {
         // ================================================================ layer-3 MMA issuer (leader; whole warp, uniform)
         if (leader) {
-            const uint32_t idesc_h[2] = {ptx::umma_idesc_bf16_f32(2 * kTM, (uint32_t)ta.n0),
-                                         ptx::umma_idesc_bf16_f32(2 * kTM, (uint32_t)(ta.n1 > 0 ? ta.n1 : 16))};
+            const uint32_t idesc_h[2] = {ptx::umma_idesc_bf16_f32(2 * kTM, (uint32_t)ta.n0, ta.f16 != 0),
+                                         ptx::umma_idesc_bf16_f32(2 * kTM, (uint32_t)(ta.n1 > 0 ? ta.n1 : 16), ta.f16 != 0)};
             TRing st;
             uint32_t acc_ph = 0;
             for (int it = 0; it < my_tiles; ++it) {
@@ -244,7 +244,7 @@ k_tail(const __grid_constant__ CUtensorMap tmapA /* row-major [rows][K3p] or blo
     } else if (warp == 2) {
         // ================================================================ layer-4 MMA issuer (leader; whole warp, uniform)
         if (leader) {
-            const uint32_t idesc4 = ptx::umma_idesc_bf16_f32(2 * kTM, (uint32_t)ta.Np);
+            const uint32_t idesc4 = ptx::umma_idesc_bf16_f32(2 * kTM, (uint32_t)ta.Np, ta.f16 != 0);
             ptx::mbar_wait_cluster(&bars[tW4Full], 0);
             const uint32_t w4_chunk = (uint32_t)(ta.Np / 2) * 128u;
             uint32_t seq = 0;
@@ -313,8 +313,8 @@ k_tail(const __grid_constant__ CUtensorMap tmapA /* row-major [rows][K3p] or blo
 #pragma unroll
                     for (int j = 0; j < 8; ++j) {
                         const float4 b = (w >= 32 || j < 4) ? b4[j] : make_float4(0.f, 0.f, 0.f, 0.f);
-                        o[2 * j] = ptx::gelu2_pack(__uint_as_float(v[4 * j]) + b.x, __uint_as_float(v[4 * j + 1]) + b.y);
-                        o[2 * j + 1] = ptx::gelu2_pack(__uint_as_float(v[4 * j + 2]) + b.z, __uint_as_float(v[4 * j + 3]) + b.w);
+                        o[2 * j] = ptx::gelu2_pack(__uint_as_float(v[4 * j]) + b.x, __uint_as_float(v[4 * j + 1]) + b.y, ta.f16 != 0);
+                        o[2 * j + 1] = ptx::gelu2_pack(__uint_as_float(v[4 * j + 2]) + b.z, __uint_as_float(v[4 * j + 3]) + b.w, ta.f16 != 0);
                     }
                 }
                 const uint32_t buf = seq & 1u, ph = (seq >> 1) & 1u;
@@ -625,6 +625,7 @@ cudaError_t launch_tail(Ctx *c, int64_t n, int64_t c0, int64_t cn, float *T, con
     ta.p = p;
     ta.ex = ex;
     ta.inv_dt = (float)(1.0 / dt);
+    ta.f16 = c->prm.precision == GPUANN_PRECISION_FP16 ? 1 : 0;
     ta.o_raw = o_raw;
     ta.o_stride = o_stride;
     ta.counters = c->counters;

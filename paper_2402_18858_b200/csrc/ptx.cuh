@@ -265,8 +265,10 @@ __device__ __forceinline__ uint64_t umma_desc_nosw_kmajor(uint32_t smem_addr, ui
 // Instruction descriptor for kind::f16 with BF16 A and B (both K-major), FP32 accumulate.
 // Bits: [4,6) D format (1 = F32), [7,10) A format (1 = BF16), [10,13) B format (1 = BF16),
 // 15 / 16 A / B major (0 = K), [17,23) N >> 3, [24,29) M >> 4.
-__host__ __device__ __forceinline__ uint32_t umma_idesc_bf16_f32(uint32_t M, uint32_t N) {
-    return (1u << 4) | (1u << 7) | (1u << 10) | ((N >> 3) << 17) | ((M >> 4) << 24);
+// f16 = true: FP16 A and B (format code 0) instead of BF16 (format code 1) -- same instruction kind, same rate.
+__host__ __device__ __forceinline__ uint32_t umma_idesc_bf16_f32(uint32_t M, uint32_t N, bool f16 = false) {
+    const uint32_t fmt = f16 ? 0u : 1u;
+    return (1u << 4) | (fmt << 7) | (fmt << 10) | ((N >> 3) << 17) | ((M >> 4) << 24);
 }
 
 // D[tmem] (+)= A[smem] * B[smem]^T; issued by ONE thread.  accumulate = 0 overwrites D.
@@ -378,10 +380,43 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
     return r;
 }
 
+// two FP32 -> packed FP16x2 (round to nearest even); `lo` lands in the low 16 bits
+__device__ __forceinline__ uint32_t pack_f16x2(float lo, float hi) {
+    uint32_t r;
+    asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+    return r;
+}
+// operand type of the tensor path chosen at run time (GPUANN_PRECISION_BF16 / _FP16): one select per pair
+__device__ __forceinline__ uint32_t pack_half2(float lo, float hi, bool f16) {
+    return f16 ? pack_f16x2(lo, hi) : pack_bf16x2(lo, hi);
+}
+
 // Two activations at once, packed to BF16x2: returns 2 GELU(v) = v + v tanh(u), u = v (c0 + c1 v^2) (tanh form, R5).
 // The factor 1/2 lives in the NEXT layer's weights (exact in BF16; api.cu scales W_l, l >= 2, of the tensor path), and
 // the polynomial runs on packed FP32x2 instructions (mul/fma.f32x2): 7 instructions per pair instead of 15.
-__device__ __forceinline__ uint32_t gelu2_pack(float v0, float v1) {
+// f16: pack to FP16x2 instead (the FP16 variant of the tensor path).
+__device__ __forceinline__ uint32_t gelu2_pack(float v0, float v1, bool f16 = false) {
+    if (f16) {
+        float a, b;
+        asm("{\n\t"
+            ".reg .b64 x, w, t, c0, c1;\n\t"
+            "mov.b64 x, {%2, %3};\n\t"
+            "mov.b64 c0, {%4, %4};\n\t"
+            "mov.b64 c1, {%5, %5};\n\t"
+            "mul.f32x2 w, x, x;\n\t"
+            "fma.rn.f32x2 t, w, c1, c0;\n\t"
+            "mul.f32x2 t, x, t;\n\t"
+            "mov.b64 {%0, %1}, t;\n\t"
+            "tanh.approx.f32 %0, %0;\n\t"
+            "tanh.approx.f32 %1, %1;\n\t"
+            "mov.b64 t, {%0, %1};\n\t"
+            "fma.rn.f32x2 t, x, t, x;\n\t"
+            "mov.b64 {%0, %1}, t;\n\t"
+            "}\n"
+            : "=&f"(a), "=&f"(b)
+            : "f"(v0), "f"(v1), "f"(0.7978845608028654f), "f"(0.0356774081363001f));
+        return pack_f16x2(a, b);
+    }
     uint32_t out;
     asm("{\n\t"
         ".reg .b64 x, w, t, c0, c1;\n\t"

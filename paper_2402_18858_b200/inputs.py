@@ -29,7 +29,7 @@ class Config:
     n_cells: int
     n_species: int
     hidden: Tuple[int, ...]
-    precision: int              # 0 = FP32 CUDA-core path, 1 = BF16 tcgen05 path
+    precision: int              # 0 = FP32 CUDA-core path, 1 = BF16 tcgen05 path, 2 = FP16 tcgen05 path
     dt: float = 1e-6            # delta t = 1 us
     newton_max_iter: int = 20
     newton_tol: float = 1e-6
@@ -61,11 +61,20 @@ CONFIGS: List[Config] = [
     Config("c3", 3, 4194304, 36, (1600, 800, 400), precision=1, dt=5e-7, newton_max_iter=10),
     Config("c4", 4, 8388608, 21, (1600, 800, 400), precision=1, T_active=600.0, mixed_field=True),
 ]
+# configs[1] / configs[2] in the half precision the paper itself infers in: same
+# seeds, states and FP32 draws; the weights are rounded to FP16 instead of BF16.  Not BASELINE.json configs (index kept).
+VARIANTS: List[Config] = [
+    Config("c1h", 1, 65536, 21, (400, 200, 100), precision=2),
+    Config("c2h", 2, 1048576, 21, (1600, 800, 400), precision=2),
+]
 
 
 def get_config(name_or_index) -> Config:
     for c in CONFIGS:
         if c.name == name_or_index or c.index == name_or_index:
+            return c
+    for c in VARIANTS:
+        if c.name == name_or_index:
             return c
     raise KeyError(name_or_index)
 
@@ -144,7 +153,7 @@ def gen_thermo(rng: np.random.Generator, Ns: int) -> Thermo:
     return Thermo(a, None, None, W)
 
 
-def gen_net(rng: np.random.Generator, sizes, bf16_weights: bool) -> Net:
+def gen_net(rng: np.random.Generator, sizes, bf16_weights: bool, f16_weights: bool = False) -> Net:
     """G3: Xavier-uniform weights, U[-1/sqrt(fan_in), 1/sqrt(fan_in)] biases, layer by layer."""
     ws, bs = [], []
     for l in range(len(sizes) - 1):
@@ -154,6 +163,8 @@ def gen_net(rng: np.random.Generator, sizes, bf16_weights: bool) -> Net:
         b = rng.uniform(-1.0 / np.sqrt(fan_in), 1.0 / np.sqrt(fan_in), fan_out).astype(np.float32)
         if bf16_weights:
             w = round_to_bf16(w)
+        if f16_weights:
+            w = w.astype(np.float16).astype(np.float32)   # round to nearest even
         ws.append(w)
         bs.append(b)
     return Net(tuple(sizes), ws, bs)
@@ -177,7 +188,7 @@ def make_problem(cfg: Config, n: Optional[int] = None, seed: Optional[int] = Non
     Ns = cfg.n_species
     state = gen_mixed_state(rng, n, Ns) if cfg.mixed_field else gen_state(rng, n, Ns)
     thermo = gen_thermo(rng, Ns)
-    net = gen_net(rng, cfg.sizes, bf16_weights=(cfg.precision == 1))
+    net = gen_net(rng, cfg.sizes, bf16_weights=(cfg.precision == 1), f16_weights=(cfg.precision == 2))
     out_mean = np.zeros(Ns, dtype=np.float32)
     out_std = np.full(Ns, cfg.sigma_out, dtype=np.float32)
     return Problem(cfg, n, state, thermo, net, out_mean, out_std)

@@ -386,3 +386,44 @@ def test_ex_outputs_two_range_thermo():
         print(f"two-range ex: {w}")
     finally:
         B.gpuann_destroy(ctx)
+
+
+# ------------------------------------------------------------------ GPUANN_PRECISION_FP16
+@pytest.mark.parametrize("name,n", [("c2h", 128 * 13 + 37), ("c1h", 128 * 40 + 5)])
+def test_fp16_variant(name, n):
+    """The same two kernels with FP16 weights and activations: gates are the BF16 ones scaled by 2^-3 (R23); the BF16 run of
+    the same cells must be the looser of the two (the variant really computes in FP16)."""
+    pr = G.prepare(I.get_config(name), n=n, seed=21)
+    ctx = G.make_ctx(pr)
+    try:
+        _, variant = B.gpuann_describe(ctx)
+        assert variant == "fp16-fused+tail"
+        g = G.run_gpu(ctx, pr)
+        ref = G.run_oracle(pr)
+        w = G.check_all_fp16(g, ref)
+        assert g.stats == (n, int((ref.flags & 1).sum()), 0)
+        print(f"{name}: {w}")
+    finally:
+        B.gpuann_destroy(ctx)
+    ctx = G.make_ctx(pr, precision=B.GPUANN_PRECISION_BF16)    # FP16-representable weights, rounded again to BF16 inside
+    try:
+        gb = G.run_gpu(ctx, pr)
+        d16 = np.abs(g.o_raw.astype(np.float64) - ref.o_raw).max()
+        db = np.abs(gb.o_raw.astype(np.float64) - ref.o_raw).max()
+        assert d16 < 0.5 * db, (d16, db)
+    finally:
+        B.gpuann_destroy(ctx)
+
+
+def test_fp16_unsupported_shapes_fail_loudly():
+    pr = G.prepare(I.get_config("c0"), n=64)     # 11-64-64-9: the fused kernel does not take H1 < 128
+    prm = B.gpuann_default_params()
+    prm.precision = B.GPUANN_PRECISION_FP16
+    ctx = B.gpuann_create(prm)
+    try:
+        with pytest.raises(B.GpuannError) as e:
+            B.gpuann_load_net(ctx, 9, pr.prob.net.sizes, pr.prob.net.weights, pr.prob.net.biases, pr.in_mean, pr.in_std,
+                              pr.prob.out_mean, pr.prob.out_std, 0.1)
+        assert e.value.status == 3
+    finally:
+        B.gpuann_destroy(ctx)

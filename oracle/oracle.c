@@ -12,6 +12,7 @@
  *   O1  Box-Cox transform of the mass fractions        PAPER.md:98-103, Eq. 7 (R1, R2)
  *   O2  input assembly {T, p, F(Y)} and z-score        PAPER.md:98 (R4)
  *   O3  fully connected GELU network                   PAPER.md:103 (R5, R6)
+ *   O3' per-species ensemble (n_nets = Ns): o_k = MLP_k(z), one D-...-1 net per species     PAPER.md:103 (R24)
  *   O4  de-normalise the output, scale by dt           PAPER.md:98 (R3)
  *   O5  inverse Box-Cox                                inverse of Eq. 7 (R7)
  *   O6  renormalise so that sum_k Y_k = 1              PAPER.md:92, 108-110 Eq. 9 (R8)
@@ -286,6 +287,10 @@ typedef struct {
     double T_min, T_max, newton_tol;
     int newton_max_iter;
     double T_active;     /* <= 0: every cell active */
+    int n_nets;          /* 0 or 1: ONE net with Ns outputs (R6).  Ns: the paper's literal architecture ("Training
+                            and prediction are individually performed for each species' mass fraction ... each MLP"; R24):
+                            Ns nets of identical shape with sizes[L] = 1; `weights` / `biases` hold net 0, net 1, ... one
+                            after the other, each laid out as for a single net; o_k is the output of net k */
 } oracle_model;
 
 /* O0..O7 for cell i.  Scratch: Ns*4 + D + 2*max_width doubles. */
@@ -320,8 +325,15 @@ static void chem_cell(const oracle_model *m, int64_t n, int64_t i, const float *
     z[1] = ((double)p[i] - (double)m->in_mean[1]) / (double)m->in_std[1];
     for (int k = 0; k < Ns; ++k)
         z[2 + k] = (y[k] - (double)m->in_mean[2 + k]) / (double)m->in_std[2 + k];
-    /* O3 */
-    mlp_forward(m->n_layers, m->sizes, m->weights, m->biases, z, o, mlp_scratch);
+    /* O3 (one net) / O3' (one net per species: the same z feeds every net; net k yields o_k) */
+    if (m->n_nets <= 1) {
+        mlp_forward(m->n_layers, m->sizes, m->weights, m->biases, z, o, mlp_scratch);
+    } else {
+        const size_t w_per_net = weight_offset(m->n_layers, m->sizes), b_per_net = bias_offset(m->n_layers, m->sizes);
+        for (int k = 0; k < Ns; ++k)
+            mlp_forward(m->n_layers, m->sizes, m->weights + (size_t)k * w_per_net, m->biases + (size_t)k * b_per_net, z,
+                        &o[k], mlp_scratch);
+    }
     /* O4, O5 */
     double S = 0.0;
     for (int k = 0; k < Ns; ++k) {
@@ -361,9 +373,9 @@ int oracle_chem_step(const oracle_model *m, int64_t n, const float *T, const flo
                      const float *h, double dt, double *T_new, double *Y_new, double *o_raw, int32_t *iters,
                      int32_t *flags)
 {
-    if (!m || n < 0 || m->n_layers < 1 || m->sizes[0] != 2 + m->n_species
-        || m->sizes[m->n_layers] != m->n_species)
-        return 1;
+    if (!m || n < 0 || m->n_layers < 1 || m->sizes[0] != 2 + m->n_species) return 1;
+    if (m->n_nets <= 1 && m->sizes[m->n_layers] != m->n_species) return 1;
+    if (m->n_nets > 1 && (m->n_nets != m->n_species || m->sizes[m->n_layers] != 1)) return 1;
     int Ns = m->n_species, D = 2 + Ns;
     size_t scratch_len = (size_t)Ns * 4 + (size_t)D + 2 * (size_t)max_width(m->n_layers, m->sizes);
     int fail = 0;

@@ -42,6 +42,7 @@ class _Model(C.Structure):
         ("T_min", C.c_double), ("T_max", C.c_double), ("newton_tol", C.c_double),
         ("newton_max_iter", C.c_int),
         ("T_active", C.c_double),
+        ("n_nets", C.c_int),
     ]
 
 
@@ -264,6 +265,9 @@ class OracleModel:
     newton_tol: float = 1e-6
     newton_max_iter: int = 20
     T_active: float = 0.0
+    # per-species ensemble (R24): sizes ends in 1 and weights / biases are lists over the Ns nets of the
+    # per-layer lists of one net
+    ensemble: bool = False
 
 
 @dataclass
@@ -281,13 +285,20 @@ class Oracle:
     def __init__(self, m: OracleModel):
         self._sizes = np.ascontiguousarray(m.sizes, dtype=np.int32)
         L = len(self._sizes) - 1
-        Ns = int(self._sizes[-1])
+        if m.ensemble:
+            Ns = int(self._sizes[0]) - 2
+            assert int(self._sizes[-1]) == 1 and len(m.weights) == Ns and len(m.biases) == Ns
+            nets_w, nets_b = m.weights, m.biases
+        else:
+            Ns = int(self._sizes[-1])
+            nets_w, nets_b = [m.weights], [m.biases]
         assert int(self._sizes[0]) == Ns + 2
-        for l in range(L):
-            assert tuple(np.shape(m.weights[l])) == (self._sizes[l + 1], self._sizes[l])
-            assert tuple(np.shape(m.biases[l])) == (self._sizes[l + 1],)
-        self._w = _f32(np.concatenate([_f32(x).ravel() for x in m.weights]))
-        self._b = _f32(np.concatenate([_f32(x).ravel() for x in m.biases]))
+        for ws, bs in zip(nets_w, nets_b):
+            for l in range(L):
+                assert tuple(np.shape(ws[l])) == (self._sizes[l + 1], self._sizes[l])
+                assert tuple(np.shape(bs[l])) == (self._sizes[l + 1],)
+        self._w = _f32(np.concatenate([_f32(x).ravel() for ws in nets_w for x in ws]))
+        self._b = _f32(np.concatenate([_f32(x).ravel() for bs in nets_b for x in bs]))
         self._im, self._is = _f32(m.in_mean), _f32(m.in_std)
         self._om, self._os = _f32(m.out_mean), _f32(m.out_std)
         assert self._im.shape == (Ns + 2,) and self._is.shape == (Ns + 2,)
@@ -300,7 +311,7 @@ class Oracle:
             _p(self._im, C.c_float), _p(self._is, C.c_float), _p(self._om, C.c_float), _p(self._os, C.c_float),
             float(m.lam), _p(self._lo, C.c_double), _p(self._hi, C.c_double), _p(self._tm, C.c_double),
             _p(self._W, C.c_double), float(m.T_min), float(m.T_max), float(m.newton_tol),
-            int(m.newton_max_iter), float(m.T_active))
+            int(m.newton_max_iter), float(m.T_active), Ns if m.ensemble else 1)
 
     def chem_step(self, T, p, Y, h, dt: float) -> OracleResult:
         lib = _load()

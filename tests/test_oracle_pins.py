@@ -619,6 +619,54 @@ def test_cp_of_the_new_state_is_dh_dT_and_the_state_equation_closes():
     assert np.allclose(d.psi, d.rho_new / st.p.astype(np.float64), rtol=1e-13)
 
 
+# ------------------------------------------------------------------ O3': per-species ensemble (R24)
+def _ensemble_from_single(m, Ns):
+    """Ns one-output nets that all carry the single net's hidden layers and row k of its last layer."""
+    import dataclasses
+    ws = [[w.copy() for w in m.weights[:-1]] + [m.weights[-1][k:k + 1].copy()] for k in range(Ns)]
+    bs = [[b.copy() for b in m.biases[:-1]] + [m.biases[-1][k:k + 1].copy()] for k in range(Ns)]
+    return dataclasses.replace(m, sizes=tuple(m.sizes[:-1]) + (1,), weights=ws, biases=bs, ensemble=True)
+
+
+def test_ensemble_with_shared_hidden_layers_equals_the_single_net():
+    pr, h, m = _small_problem(n=96)
+    st = pr.state
+    Ns = pr.cfg.n_species
+    r1 = oracle.Oracle(m).chem_step(st.T, st.p, st.Y, h, 1e-6)
+    r2 = oracle.Oracle(_ensemble_from_single(m, Ns)).chem_step(st.T, st.p, st.Y, h, 1e-6)
+    assert np.array_equal(r1.o_raw, r2.o_raw) and np.array_equal(r1.Y_new, r2.Y_new) and np.array_equal(r1.T_new, r2.T_new)
+
+
+def test_ensemble_output_k_is_net_k_alone_and_matches_numpy():
+    """Net j != k does not enter o_k (bit-identical after perturbing net j), net k does; and o_k equals the numpy / scipy
+    forward pass of net k on the independently built z.  Catches nets indexed by the wrong stride or all outputs from net 0."""
+    pr, h, m = _small_problem(n=16)
+    st, cfg = pr.state, pr.cfg
+    Ns = cfg.n_species
+    rng = np.random.default_rng(11)
+    sizes = tuple(m.sizes[:-1]) + (1,)
+    ws = [[rng.uniform(-0.4, 0.4, (sizes[l + 1], sizes[l])).astype(np.float32) for l in range(len(sizes) - 1)] for _ in range(Ns)]
+    bs = [[rng.uniform(-0.3, 0.3, sizes[l + 1]).astype(np.float32) for l in range(len(sizes) - 1)] for _ in range(Ns)]
+    import dataclasses
+    me = dataclasses.replace(m, sizes=sizes, weights=ws, biases=bs, ensemble=True)
+    r = oracle.Oracle(me).chem_step(st.T, st.p, st.Y, h, 1e-6)
+    x = np.vstack([st.T.astype(np.float64), st.p.astype(np.float64),
+                   special.boxcox(np.maximum(st.Y.astype(np.float64), 0.0), cfg.lam)])
+    z = (x - m.in_mean.astype(np.float64)[:, None]) / m.in_std.astype(np.float64)[:, None]
+    for k in range(Ns):
+        a = z
+        for l in range(len(sizes) - 1):
+            a = ws[k][l].astype(np.float64) @ a + bs[k][l].astype(np.float64)[:, None]
+            if l < len(sizes) - 2:
+                a = a * special.ndtr(a)
+        assert np.allclose(r.o_raw[k], a[0], rtol=1e-12, atol=1e-13)
+    ws2 = [[w.copy() for w in net] for net in ws]
+    ws2[3][0][:] += 0.25                                        # perturb net 3 only
+    r2 = oracle.Oracle(dataclasses.replace(me, weights=ws2)).chem_step(st.T, st.p, st.Y, h, 1e-6)
+    others = [k for k in range(Ns) if k != 3]
+    assert np.array_equal(r2.o_raw[others], r.o_raw[others]) and not np.array_equal(r2.o_raw[3], r.o_raw[3])
+
+
 def test_paper_speedup_arithmetic():
     """context numbers in BASELINE.md are self-consistent (ratio = 32/(1 - reduction))."""
     for red, ratio in read_golden("speedup_arithmetic.txt"):

@@ -106,6 +106,19 @@ int gpuann_load_net(gpuann_ctx *ctx, int n_species, int n_layers, const int *siz
                     const float *in_mean, const float *in_std,
                     const float *out_mean, const float *out_std, double lambda);
 
+/* The paper's literal architecture ("Training and prediction are individually performed for each species'
+ * mass fraction ... The architecture of each MLP"; R24): Ns nets of ONE shape with a
+ * single output each, all fed by the same z; net k yields o_k, everything after S3 is unchanged.
+ *   sizes    HOST int[L+1]: sizes[0] = 2 + Ns, hidden widths, sizes[L] = 1
+ *   weights  HOST, Ns*L pointers: layer l of net k at weights[k*L + l], row-major [sizes[l+1]][sizes[l]]; biases likewise
+ * Tensor path only (BF16 or FP16 context) and only shapes the fused + tail kernels run (L = 4, first hidden layer >= 128,
+ * last hidden layer <= 416): UNSUPPORTED otherwise.  One step is Ns x (fused kernel + tail kernel) + one update kernel;
+ * gpuann_chem_step_ex's optional outputs are not available with an ensemble.  Replaces a net loaded earlier. */
+int gpuann_load_net_ensemble(gpuann_ctx *ctx, int n_species, int n_layers, const int *sizes,
+                             const float *const *weights, const float *const *biases,
+                             const float *in_mean, const float *in_std,
+                             const float *out_mean, const float *out_std, double lambda);
+
 /* Loads the thermodynamic table of S7 ("high-order temperature polynomials"; R9).
  *   nasa_lo  HOST double[Ns][7]: a1..a7 of the low-temperature range
  *   nasa_hi  HOST double[Ns][7] or NULL (= one range: nasa_lo is used at every T)

@@ -26,7 +26,7 @@ GPUANN_PRECISION_FP16 = 2
 
 # every symbol include/gpuann.h declares (tests check that the library exports all of them)
 SYMBOLS = [
-    "gpuann_default_params", "gpuann_create", "gpuann_load_net", "gpuann_load_thermo", "gpuann_chem_step",
+    "gpuann_default_params", "gpuann_create", "gpuann_load_net", "gpuann_load_net_ensemble", "gpuann_load_thermo", "gpuann_chem_step",
     "gpuann_chem_step_ex",
     "gpuann_chem_step_host", "gpuann_debug_forward", "gpuann_get_stats", "gpuann_reset_stats", "gpuann_enthalpy",
     "gpuann_input_moments", "gpuann_launch_count", "gpuann_timing_enable", "gpuann_timing_read",
@@ -69,6 +69,8 @@ def lib() -> C.CDLL:
     L.gpuann_create.argtypes = [C.POINTER(gpuann_params), C.POINTER(vp)]
     L.gpuann_load_net.restype = C.c_int
     L.gpuann_load_net.argtypes = [vp, C.c_int, C.c_int, C.POINTER(C.c_int), fpp, fpp, vp, vp, vp, vp, dbl]
+    L.gpuann_load_net_ensemble.restype = C.c_int
+    L.gpuann_load_net_ensemble.argtypes = [vp, C.c_int, C.c_int, C.POINTER(C.c_int), fpp, fpp, vp, vp, vp, vp, dbl]
     L.gpuann_load_thermo.restype = C.c_int
     L.gpuann_load_thermo.argtypes = [vp, C.c_int, vp, vp, vp, vp]
     L.gpuann_chem_step.restype = C.c_int
@@ -159,6 +161,30 @@ def gpuann_load_net(ctx: int, n_species: int, sizes: Sequence[int], weights: Seq
     im, isd, om, osd = _f32(in_mean), _f32(in_std), _f32(out_mean), _f32(out_std)
     st = lib().gpuann_load_net(ctx, int(n_species), Lw, sz.ctypes.data_as(C.POINTER(C.c_int)), wp, bp,
                                _ptr(im), _ptr(isd), _ptr(om), _ptr(osd), float(lam))
+    _check(st, ctx)
+
+
+def gpuann_load_net_ensemble(ctx: int, n_species: int, sizes: Sequence[int], weights, biases, in_mean, in_std, out_mean,
+                             out_std, lam: float) -> None:
+    """weights[k][l], biases[k][l]: layer l of the net of species k (every net has the shape `sizes`, sizes[-1] == 1)."""
+    sz = np.ascontiguousarray(sizes, dtype=np.int32)
+    Lw = len(sz) - 1
+    if len(weights) != n_species or len(biases) != n_species:
+        raise ValueError("one list of layers per species")
+    ws = [[_f32(w) for w in net] for net in weights]
+    bs = [[_f32(b) for b in net] for net in biases]
+    for k in range(n_species):
+        if len(ws[k]) != Lw or len(bs[k]) != Lw:
+            raise ValueError("every net needs len(sizes) - 1 layers")
+        for l in range(Lw):
+            if ws[k][l].shape != (sz[l + 1], sz[l]) or bs[k][l].shape != (sz[l + 1],):
+                raise ValueError(f"net {k} layer {l}: weights must be [out][in] = {(sz[l + 1], sz[l])}, biases [out]")
+    fp = C.POINTER(C.c_float)
+    wp = (fp * (Lw * n_species))(*[w.ctypes.data_as(fp) for net in ws for w in net])
+    bp = (fp * (Lw * n_species))(*[b.ctypes.data_as(fp) for net in bs for b in net])
+    im, isd, om, osd = _f32(in_mean), _f32(in_std), _f32(out_mean), _f32(out_std)
+    st = lib().gpuann_load_net_ensemble(ctx, int(n_species), Lw, sz.ctypes.data_as(C.POINTER(C.c_int)), wp, bp,
+                                        _ptr(im), _ptr(isd), _ptr(om), _ptr(osd), float(lam))
     _check(st, ctx)
 
 

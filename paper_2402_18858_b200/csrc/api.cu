@@ -76,14 +76,28 @@ void free_net(Ctx *c) {
     cudaFree(c->b32);
     c->w32 = c->b32 = nullptr;
     c->w32_count = c->b32_count = 0;
-    for (int l = 0; l < kMaxLayers; ++l) {
-        cudaFree(c->lay[l].W);
-        cudaFree(c->lay[l].bias);
-        c->lay[l] = LayerBf16{};
+    auto free_sub = [](SubNet &sn) {
+        for (int l = 0; l < kMaxLayers; ++l) {
+            cudaFree(sn.lay[l].W);
+            cudaFree(sn.lay[l].bias);
+        }
+        cudaFree(sn.fused.W1p);
+        sn = SubNet{};
+    };
+    {   // the thermo table of the tail kernel survives a reload of the net (gpuann_load_thermo may have come first)
+        const TailThermo th = c->net0.tail.args.th;
+        const int two = c->net0.tail.args.two_ranges;
+        TailArgs keep = c->net0.tail.args;
+        free_sub(c->net0);
+        std::memcpy(c->net0.tail.args.hhf, keep.hhf, sizeof(keep.hhf));
+        std::memcpy(c->net0.tail.args.cpf, keep.cpf, sizeof(keep.cpf));
+        std::memcpy(c->net0.tail.args.invW, keep.invW, sizeof(keep.invW));
+        c->net0.tail.args.th = th;
+        c->net0.tail.args.two_ranges = two;
     }
-    cudaFree(c->fused.W1p);
-    c->fused = FusedNet{};
-    c->tail.on = false;
+    for (SubNet &sn : c->ens) free_sub(sn);
+    c->ens.clear();
+    c->cur = &c->net0;
     cudaFree(c->act[0]);
     cudaFree(c->act[1]);
     cudaFree(c->o_buf);
@@ -96,6 +110,159 @@ void free_net(Ctx *c) {
 }
 
 bool finite_f(float x) { return std::isfinite(x); }
+
+
+// which kernels a net of these sizes runs, and its scratch: sets c->chunk, allocates the activation buffers (shared by all
+// nets of an ensemble) and, when no tail kernel consumes the raw output in place (or `need_obuf`), the o buffer
+int plan_and_alloc(Ctx *c, int n_species, int n_layers, const int *sizes, bool need_obuf) {
+    const bool f16 = c->prm.precision == GPUANN_PRECISION_FP16;
+    const bool fused = n_layers >= 3 && fused_supported(sizes[0], sizes[1], pad16(sizes[2]));
+    const bool tail = n_layers >= (fused ? 4 : 2) &&
+                      tail_supported(pad16(sizes[n_layers - 2]), pad16(sizes[n_layers - 1]), sizes[n_layers]);
+    if (f16 && !(fused && tail && n_layers == 4))
+        return fail(c, GPUANN_ERR_UNSUPPORTED, "gpuann_load_net: GPUANN_PRECISION_FP16 needs a net the fused + tail kernels run (4 weight matrices)");
+    int64_t chunk = c->prm.chunk_cells > 0 ? c->prm.chunk_cells : (int64_t)c->sm_count * 128 * (fused ? 56 : 1);
+    chunk = (chunk + 127) / 128 * 128;
+    c->chunk = chunk;
+    int maxKp = 0;
+    for (int l = 0; l < n_layers; ++l)
+        if (!fused || l >= 2) maxKp = pad16(sizes[l]) > maxKp ? pad16(sizes[l]) : maxKp;
+    // activation scratch: ping-pong buffers [chunk][maxKp]; with the fused kernel in front and the tail kernel behind
+    // only ONE of them is ever used (h2), and the raw output never leaves the SM
+    c->act_elems = (size_t)chunk * (size_t)maxKp;
+    const bool one_buffer = fused && tail && n_layers == 4;
+    for (int b = 0; b < (one_buffer ? 1 : 2); ++b) {
+        CU_TRY(c, cudaMalloc(&c->act[b], c->act_elems * sizeof(__nv_bfloat16)), "cudaMalloc(activations)");
+        CU_TRY(c, cudaMemset(c->act[b], 0, c->act_elems * sizeof(__nv_bfloat16)), "cudaMemset(activations)");
+    }
+    if (!tail || need_obuf) {
+        CU_TRY(c, cudaMalloc(&c->o_buf, (size_t)n_species * chunk * sizeof(float)), "cudaMalloc(o_buf)");
+        CU_TRY(c, cudaMemset(c->o_buf, 0, (size_t)n_species * chunk * sizeof(float)), "cudaMemset(o_buf)");
+    }
+    return GPUANN_OK;
+}
+
+// pads, rounds (RNE) and uploads one net of the tensor path and encodes its tensor maps (against the context's shared
+// activation buffers: plan_and_alloc first).  n_out = sizes[n_layers].  *mac_out: MACs issued per cell including padding.
+int build_subnet(Ctx *c, SubNet &sn, int n_out, int n_layers, const int *sizes, const float *const *weights,
+                 const float *const *biases, int64_t *mac_out) {
+    const PreParams &pre = c->pre;
+    const PostParams &po = c->post;
+    const int64_t chunk = c->chunk;
+    sn.n_out = n_out;
+    const bool f16 = c->prm.precision == GPUANN_PRECISION_FP16;
+    auto to_half = [f16](float v) { return f16 ? f32_to_f16_rne(v) : f32_to_bf16_rne(v); };
+    const bool fused = n_layers >= 3 && fused_supported(sizes[0], sizes[1], pad16(sizes[2]));
+    const bool tail = n_layers >= (fused ? 4 : 2) &&
+                      tail_supported(pad16(sizes[n_layers - 2]), pad16(sizes[n_layers - 1]), n_out);
+    int64_t mac = 0;
+    for (int l = 0; l < n_layers; ++l) {
+        LayerBf16 &ly = sn.lay[l];
+        ly.K = sizes[l];
+        ly.N = sizes[l + 1];
+        ly.Kp = pad16(ly.K);
+        ly.Np = pad16(ly.N);
+        ly.tiles_n = (ly.Np + 415) / 416;
+        ly.n_tile = pad16((ly.Np + ly.tiles_n - 1) / ly.tiles_n);
+        ly.tiles_n = (ly.Np + ly.n_tile - 1) / ly.n_tile;
+        ly.n0 = ly.n_tile > 256 ? pad16((ly.n_tile + 1) / 2) : 0;
+        mac += (int64_t)ly.Kp * ly.Np;
+        std::vector<uint16_t> hw((size_t)ly.Np * ly.Kp, 0);
+        std::vector<float> hb((size_t)ly.Np, 0.f);
+        // every hidden activation is stored as 2 GELU(.) (ptx::gelu2_pack): its consumer W_l, l >= 1, carries the 1/2
+        const float wscale = l >= 1 ? 0.5f : 1.f;
+        for (int j = 0; j < ly.N; ++j) {
+            for (int i = 0; i < ly.K; ++i) hw[(size_t)j * ly.Kp + i] = to_half(wscale * weights[l][(size_t)j * ly.K + i]);
+            hb[j] = biases[l][j];
+        }
+        CU_TRY(c, cudaMalloc(&ly.W, hw.size() * sizeof(uint16_t)), "cudaMalloc(W bf16)");
+        CU_TRY(c, cudaMalloc(&ly.bias, hb.size() * sizeof(float)), "cudaMalloc(bias)");
+        CU_TRY(c, cudaMemcpy(ly.W, hw.data(), hw.size() * sizeof(uint16_t), cudaMemcpyHostToDevice), "cudaMemcpy(W)");
+        CU_TRY(c, cudaMemcpy(ly.bias, hb.data(), hb.size() * sizeof(float), cudaMemcpyHostToDevice), "cudaMemcpy(bias)");
+        std::string terr;
+        if (!encode_tmap_bf16(&ly.tmapW, ly.W, (uint64_t)ly.Kp, (uint64_t)ly.Np, (uint64_t)ly.Kp * 2, (uint32_t)(ly.n0 > 0 ? ly.n0 : ly.n_tile), &terr))
+            return fail(c, GPUANN_ERR_CUDA, "gpuann_load_net: " + terr);
+    }
+    if (fused) {
+        FusedNet &fn = sn.fused;
+        const int D = sizes[0], H1 = sizes[1];
+        fused_plan(sn.lay[1].Np, &fn.n_pass, &fn.pass_w, &fn.n0, &fn.n1);
+        // W1 padded to K = 64 with the bias in two extra columns: b1 = hi + lo, both BF16, multiplied by the
+        // constant-1 features z[D], z[D+1] the kernel appends (bias error <= 2^-17 |b1|)
+        const int H1p = (H1 + 63) / 64 * 64;  // rows up to the next multiple of 64 stay zero: h1 = 0 there (k_fused.cu)
+        std::vector<uint16_t> w1((size_t)H1p * 64, 0);
+        for (int j = 0; j < H1; ++j) {
+            for (int i = 0; i < D; ++i) w1[(size_t)j * 64 + i] = to_half(weights[0][(size_t)j * D + i]);
+            const float b = biases[0][j];
+            const uint16_t hi = to_half(b);
+            float hf;
+            if (f16) {
+                hf = f16_bits_to_f32(hi);
+            } else {
+                uint32_t hbits = (uint32_t)hi << 16;
+                std::memcpy(&hf, &hbits, 4);
+            }
+            w1[(size_t)j * 64 + D] = hi;
+            w1[(size_t)j * 64 + D + 1] = to_half(b - hf);
+        }
+        CU_TRY(c, cudaMalloc(&fn.W1p, w1.size() * sizeof(uint16_t)), "cudaMalloc(W1 padded)");
+        CU_TRY(c, cudaMemcpy(fn.W1p, w1.data(), w1.size() * sizeof(uint16_t), cudaMemcpyHostToDevice), "cudaMemcpy(W1 padded)");
+        std::string terr;
+        const LayerBf16 &l2 = sn.lay[1];
+        // boxes are a CTA's HALF of a stage: the pair's MMAs (cta_group::2) read half of B from each CTA (k_fused.cu)
+        if (!encode_tmap_bf16(&fn.tmapW1, fn.W1p, 64, (uint64_t)H1p, 128, 16, &terr) ||
+            !encode_tmap_bf16(&fn.tmapW2a, l2.W, (uint64_t)l2.Kp, (uint64_t)l2.Np, (uint64_t)l2.Kp * 2, (uint32_t)(fn.n0 / 2), &terr) ||
+            !encode_tmap_bf16(&fn.tmapW2b, l2.W, (uint64_t)l2.Kp, (uint64_t)l2.Np, (uint64_t)l2.Kp * 2,
+                              (uint32_t)(fn.n1 > 0 ? fn.n1 / 2 : 8), &terr))
+            return fail(c, GPUANN_ERR_CUDA, "gpuann_load_net: " + terr);
+        fn.on = true;
+        // MACs issued: layer 1 once per pass over 16 * Kz columns, layer 2 over n_pass * pass_w columns
+        const int Kz16 = ((D + 2 + 15) / 16) * 16;
+        mac += (int64_t)fn.n_pass * H1p * Kz16 - (int64_t)sn.lay[0].Kp * sn.lay[0].Np;
+        mac += (int64_t)H1p * (int64_t)fn.n_pass * fn.pass_w - (int64_t)l2.Kp * l2.Np;
+    }
+    const bool one_buffer = fused && tail && n_layers == 4;
+    for (int l = fused ? 2 : 0; l < n_layers; ++l) {
+        LayerBf16 &ly = sn.lay[l];
+        std::string terr;
+        if (!encode_tmap_bf16(&ly.tmapA, c->act[l & 1], (uint64_t)ly.Kp, (uint64_t)chunk, (uint64_t)ly.Kp * 2, 128, &terr))
+            return fail(c, GPUANN_ERR_CUDA, "gpuann_load_net: " + terr);
+    }
+    if (tail) {
+        TailNet &tn = sn.tail;
+        const LayerBf16 &l3 = sn.lay[n_layers - 2], &l4 = sn.lay[n_layers - 1];
+        TailArgs &ta = tn.args;
+        ta.Ns = n_out;
+        ta.Np = l4.Np;
+        ta.K3p = l3.Kp;
+        ta.H3p = l3.Np;
+        tail_plan(l3.Np, &ta.n0, &ta.n1);
+        ta.bias3 = l3.bias;
+        ta.newton_max_iter = po.newton_max_iter;
+        ta.inv_lambda_int = po.inv_lambda_int;
+        ta.lambda_zero = po.lambda_zero;
+        ta.lambda = pre.lambda;
+        ta.inv_lambda = pre.inv_lambda;
+        ta.newton_tol = po.newton_tol;
+        ta.T_min = po.T_min;
+        ta.T_max = po.T_max;
+        for (int k = 0; k < kTailMaxNs; ++k) ta.b4[k] = k < n_out ? biases[n_layers - 1][k] : 0.f;
+        std::string terr;
+        if (!encode_tmap_bf16(&tn.tmapW3a, l3.W, (uint64_t)l3.Kp, (uint64_t)l3.Np, (uint64_t)l3.Kp * 2, (uint32_t)(ta.n0 / 2), &terr) ||
+            !encode_tmap_bf16(&tn.tmapW3b, l3.W, (uint64_t)l3.Kp, (uint64_t)l3.Np, (uint64_t)l3.Kp * 2,
+                              (uint32_t)(ta.n1 > 0 ? ta.n1 / 2 : 8), &terr) ||
+            !encode_tmap_bf16(&tn.tmapW4, l4.W, (uint64_t)l4.Kp, (uint64_t)l4.Np, (uint64_t)l4.Kp * 2, (uint32_t)(l4.Np / 2), &terr))
+            return fail(c, GPUANN_ERR_CUDA, "gpuann_load_net: " + terr);
+        // fused kernel directly in front: h2 travels in the blocked layout (common.cuh, FusedNet)
+        ta.a_blocked = one_buffer ? 1 : 0;
+        sn.fused.h2_blocked = one_buffer;
+        if (one_buffer && !encode_tmap_bf16_linear(&tn.tmapAb, c->act[0], (uint64_t)chunk * (uint64_t)l3.Kp, &terr))
+            return fail(c, GPUANN_ERR_CUDA, "gpuann_load_net: " + terr);
+        tn.on = true;
+    }
+    if (mac_out) *mac_out = mac;
+    return GPUANN_OK;
+}
 
 }  // namespace
 
@@ -171,34 +338,35 @@ int gpuann_create(const gpuann_params *params, gpuann_ctx **out) {
     return GPUANN_OK;
 }
 
-int gpuann_load_net(gpuann_ctx *c, int n_species, int n_layers, const int *sizes, const float *const *weights,
-                    const float *const *biases, const float *in_mean, const float *in_std, const float *out_mean,
-                    const float *out_std, double lambda) {
-    if (!c) return fail(nullptr, GPUANN_ERR_INVALID_ARG, "gpuann_load_net: ctx is NULL");
+// validation + the parameter blocks every path shares (S1-S2 statistics, S4-S7 constants); frees the previous net
+static int load_prologue(gpuann_ctx *c, const char *fn, int n_species, int n_layers, const int *sizes, int n_out, int n_nets,
+                         const float *const *weights, const float *const *biases, const float *in_mean,
+                         const float *in_std, const float *out_mean, const float *out_std, double lambda) {
+    if (!c) return fail(nullptr, GPUANN_ERR_INVALID_ARG, std::string(fn) + ": ctx is NULL");
     if (!sizes || !weights || !biases || !in_mean || !in_std || !out_mean || !out_std)
-        return fail(c, GPUANN_ERR_INVALID_ARG, "gpuann_load_net: NULL argument");
-    if (n_species < 1 || n_layers < 1) return fail(c, GPUANN_ERR_INVALID_ARG, "gpuann_load_net: n_species, n_layers must be >= 1");
+        return fail(c, GPUANN_ERR_INVALID_ARG, std::string(fn) + ": NULL argument");
+    if (n_species < 1 || n_layers < 1) return fail(c, GPUANN_ERR_INVALID_ARG, std::string(fn) + ": n_species, n_layers must be >= 1");
     if (n_species > GPUANN_MAX_SPECIES || n_layers > GPUANN_MAX_LAYERS)
-        return fail(c, GPUANN_ERR_UNSUPPORTED, "gpuann_load_net: n_species > 64 or n_layers > 8");
-    if (sizes[0] != n_species + 2 || sizes[n_layers] != n_species)
-        return fail(c, GPUANN_ERR_INVALID_ARG, "gpuann_load_net: sizes[0] must be 2+Ns and sizes[L] must be Ns");
+        return fail(c, GPUANN_ERR_UNSUPPORTED, std::string(fn) + ": n_species > 64 or n_layers > 8");
+    if (sizes[0] != n_species + 2 || sizes[n_layers] != n_out)
+        return fail(c, GPUANN_ERR_INVALID_ARG, std::string(fn) + ": sizes[0] must be 2+Ns and sizes[L] must be " + (n_out == 1 ? "1" : "Ns"));
     int maxw = 0;
     for (int l = 0; l <= n_layers; ++l) {
-        if (sizes[l] < 1) return fail(c, GPUANN_ERR_INVALID_ARG, "gpuann_load_net: layer width < 1");
-        if (sizes[l] > GPUANN_MAX_WIDTH) return fail(c, GPUANN_ERR_UNSUPPORTED, "gpuann_load_net: layer width > 4096");
+        if (sizes[l] < 1) return fail(c, GPUANN_ERR_INVALID_ARG, std::string(fn) + ": layer width < 1");
+        if (sizes[l] > GPUANN_MAX_WIDTH) return fail(c, GPUANN_ERR_UNSUPPORTED, std::string(fn) + ": layer width > 4096");
         maxw = sizes[l] > maxw ? sizes[l] : maxw;
     }
-    for (int l = 0; l < n_layers; ++l)
-        if (!weights[l] || !biases[l]) return fail(c, GPUANN_ERR_INVALID_ARG, "gpuann_load_net: NULL weight or bias pointer");
+    for (int l = 0; l < n_layers * n_nets; ++l)
+        if (!weights[l] || !biases[l]) return fail(c, GPUANN_ERR_INVALID_ARG, std::string(fn) + ": NULL weight or bias pointer");
     for (int j = 0; j < n_species + 2; ++j)
         if (!finite_f(in_mean[j]) || !finite_f(in_std[j]) || !(in_std[j] > 0.f))
-            return fail(c, GPUANN_ERR_INVALID_ARG, "gpuann_load_net: in_mean must be finite and in_std finite and > 0");
+            return fail(c, GPUANN_ERR_INVALID_ARG, std::string(fn) + ": in_mean must be finite and in_std finite and > 0");
     for (int k = 0; k < n_species; ++k)
         if (!finite_f(out_mean[k]) || !finite_f(out_std[k]))
-            return fail(c, GPUANN_ERR_INVALID_ARG, "gpuann_load_net: out_mean / out_std must be finite");
-    if (!(lambda >= 0.0) || !std::isfinite(lambda)) return fail(c, GPUANN_ERR_INVALID_ARG, "gpuann_load_net: lambda must be >= 0");
+            return fail(c, GPUANN_ERR_INVALID_ARG, std::string(fn) + ": out_mean / out_std must be finite");
+    if (!(lambda >= 0.0) || !std::isfinite(lambda)) return fail(c, GPUANN_ERR_INVALID_ARG, std::string(fn) + ": lambda must be >= 0");
     if (c->thermo_loaded && c->thermo_Ns != n_species)
-        return fail(c, GPUANN_ERR_INVALID_ARG, "gpuann_load_net: n_species differs from the loaded thermo table");
+        return fail(c, GPUANN_ERR_INVALID_ARG, std::string(fn) + ": n_species differs from the loaded thermo table");
 
     DeviceGuard g(c->device);
     cudaDeviceSynchronize();
@@ -239,6 +407,23 @@ int gpuann_load_net(gpuann_ctx *c, int n_species, int n_layers, const int *sizes
         po.out_std[k] = out_std[k];
     }
 
+    return GPUANN_OK;
+}
+
+int gpuann_load_net(gpuann_ctx *c, int n_species, int n_layers, const int *sizes, const float *const *weights,
+                    const float *const *biases, const float *in_mean, const float *in_std, const float *out_mean,
+                    const float *out_std, double lambda) {
+    if (!c) return fail(nullptr, GPUANN_ERR_INVALID_ARG, "gpuann_load_net: ctx is NULL");
+    {
+        const int rc0 = load_prologue(c, "gpuann_load_net", n_species, n_layers, sizes, n_species, 1, weights, biases, in_mean,
+                                      in_std, out_mean, out_std, lambda);
+        if (rc0 != GPUANN_OK) return rc0;
+    }
+    DeviceGuard g(c->device);
+    PreParams &pre = c->pre;
+    PostParams &po = c->post;
+    (void)pre;
+    (void)po;
     if (c->prm.precision == GPUANN_PRECISION_FP32) {
         size_t wc = 0, bc = 0;
         for (int l = 0; l < n_layers; ++l) {
@@ -269,142 +454,48 @@ int gpuann_load_net(gpuann_ctx *c, int n_species, int n_layers, const int *sizes
         return GPUANN_OK;
     }
 
-    // ---- BF16 tensor path: pad, round (RNE), upload, encode the tensor maps
-    // variant: "bf16-fused" (S1 + S2 + layers 1-2 in one kernel, k_fused.cu) when the shapes allow it, else
-    // "bf16-layerwise"
+    // ---- tensor path
+    int rc = plan_and_alloc(c, n_species, n_layers, sizes, false);
+    if (rc != GPUANN_OK) return rc;
+    rc = build_subnet(c, c->net0, n_species, n_layers, sizes, weights, biases, &c->issued_mac_per_cell);
+    if (rc != GPUANN_OK) return rc;
+    c->cur = &c->net0;
     const bool f16 = c->prm.precision == GPUANN_PRECISION_FP16;
-    auto to_half = [f16](float v) { return f16 ? f32_to_f16_rne(v) : f32_to_bf16_rne(v); };
-    const bool fused = n_layers >= 3 && fused_supported(sizes[0], sizes[1], pad16(sizes[2]));
-    // "+tail": the last two layers and the update S4-S8 in one kernel (k_tail.cu); needs a layer in front of them
-    // (the fused kernel or a GEMM) that leaves their input in an activation buffer
-    const bool tail = n_layers >= (fused ? 4 : 2) &&
-                      tail_supported(pad16(sizes[n_layers - 2]), pad16(sizes[n_layers - 1]), n_species);
-    if (f16 && !(fused && tail && n_layers == 4))
-        return fail(c, GPUANN_ERR_UNSUPPORTED, "gpuann_load_net: GPUANN_PRECISION_FP16 needs a net the fused + tail kernels run (4 weight matrices)");
-    int64_t chunk = c->prm.chunk_cells > 0 ? c->prm.chunk_cells : (int64_t)c->sm_count * 128 * (fused ? 56 : 1);
-    chunk = (chunk + 127) / 128 * 128;
-    c->chunk = chunk;
-    int maxKp = 0;
-    int64_t mac = 0;
-    for (int l = 0; l < n_layers; ++l) {
-        LayerBf16 &ly = c->lay[l];
-        ly.K = sizes[l];
-        ly.N = sizes[l + 1];
-        ly.Kp = pad16(ly.K);
-        ly.Np = pad16(ly.N);
-        ly.tiles_n = (ly.Np + 415) / 416;
-        ly.n_tile = pad16((ly.Np + ly.tiles_n - 1) / ly.tiles_n);
-        ly.tiles_n = (ly.Np + ly.n_tile - 1) / ly.n_tile;
-        ly.n0 = ly.n_tile > 256 ? pad16((ly.n_tile + 1) / 2) : 0;
-        if (!fused || l >= 2) maxKp = ly.Kp > maxKp ? ly.Kp : maxKp;
-        mac += (int64_t)ly.Kp * ly.Np;
-        std::vector<uint16_t> hw((size_t)ly.Np * ly.Kp, 0);
-        std::vector<float> hb((size_t)ly.Np, 0.f);
-        // every hidden activation is stored as 2 GELU(.) (ptx::gelu2_pack): its consumer W_l, l >= 1, carries the 1/2
-        const float wscale = l >= 1 ? 0.5f : 1.f;
-        for (int j = 0; j < ly.N; ++j) {
-            for (int i = 0; i < ly.K; ++i) hw[(size_t)j * ly.Kp + i] = to_half(wscale * weights[l][(size_t)j * ly.K + i]);
-            hb[j] = biases[l][j];
-        }
-        CU_TRY(c, cudaMalloc(&ly.W, hw.size() * sizeof(uint16_t)), "cudaMalloc(W bf16)");
-        CU_TRY(c, cudaMalloc(&ly.bias, hb.size() * sizeof(float)), "cudaMalloc(bias)");
-        CU_TRY(c, cudaMemcpy(ly.W, hw.data(), hw.size() * sizeof(uint16_t), cudaMemcpyHostToDevice), "cudaMemcpy(W)");
-        CU_TRY(c, cudaMemcpy(ly.bias, hb.data(), hb.size() * sizeof(float), cudaMemcpyHostToDevice), "cudaMemcpy(bias)");
-        std::string terr;
-        if (!encode_tmap_bf16(&ly.tmapW, ly.W, (uint64_t)ly.Kp, (uint64_t)ly.Np, (uint64_t)ly.Kp * 2, (uint32_t)(ly.n0 > 0 ? ly.n0 : ly.n_tile), &terr))
-            return fail(c, GPUANN_ERR_CUDA, "gpuann_load_net: " + terr);
-    }
-    if (fused) {
-        FusedNet &fn = c->fused;
-        const int D = sizes[0], H1 = sizes[1];
-        fused_plan(c->lay[1].Np, &fn.n_pass, &fn.pass_w, &fn.n0, &fn.n1);
-        // W1 padded to K = 64 with the bias in two extra columns: b1 = hi + lo, both BF16, multiplied by the
-        // constant-1 features z[D], z[D+1] the kernel appends (bias error <= 2^-17 |b1|)
-        const int H1p = (H1 + 63) / 64 * 64;  // rows up to the next multiple of 64 stay zero: h1 = 0 there (k_fused.cu)
-        std::vector<uint16_t> w1((size_t)H1p * 64, 0);
-        for (int j = 0; j < H1; ++j) {
-            for (int i = 0; i < D; ++i) w1[(size_t)j * 64 + i] = to_half(weights[0][(size_t)j * D + i]);
-            const float b = biases[0][j];
-            const uint16_t hi = to_half(b);
-            float hf;
-            if (f16) {
-                hf = f16_bits_to_f32(hi);
-            } else {
-                uint32_t hbits = (uint32_t)hi << 16;
-                std::memcpy(&hf, &hbits, 4);
-            }
-            w1[(size_t)j * 64 + D] = hi;
-            w1[(size_t)j * 64 + D + 1] = to_half(b - hf);
-        }
-        CU_TRY(c, cudaMalloc(&fn.W1p, w1.size() * sizeof(uint16_t)), "cudaMalloc(W1 padded)");
-        CU_TRY(c, cudaMemcpy(fn.W1p, w1.data(), w1.size() * sizeof(uint16_t), cudaMemcpyHostToDevice), "cudaMemcpy(W1 padded)");
-        std::string terr;
-        const LayerBf16 &l2 = c->lay[1];
-        // boxes are a CTA's HALF of a stage: the pair's MMAs (cta_group::2) read half of B from each CTA (k_fused.cu)
-        if (!encode_tmap_bf16(&fn.tmapW1, fn.W1p, 64, (uint64_t)H1p, 128, 16, &terr) ||
-            !encode_tmap_bf16(&fn.tmapW2a, l2.W, (uint64_t)l2.Kp, (uint64_t)l2.Np, (uint64_t)l2.Kp * 2, (uint32_t)(fn.n0 / 2), &terr) ||
-            !encode_tmap_bf16(&fn.tmapW2b, l2.W, (uint64_t)l2.Kp, (uint64_t)l2.Np, (uint64_t)l2.Kp * 2,
-                              (uint32_t)(fn.n1 > 0 ? fn.n1 / 2 : 8), &terr))
-            return fail(c, GPUANN_ERR_CUDA, "gpuann_load_net: " + terr);
-        fn.on = true;
-        // MACs issued: layer 1 once per pass over 16 * Kz columns, layer 2 over n_pass * pass_w columns
-        const int Kz16 = ((D + 2 + 15) / 16) * 16;
-        mac += (int64_t)fn.n_pass * H1p * Kz16 - (int64_t)c->lay[0].Kp * c->lay[0].Np;
-        mac += (int64_t)H1p * (int64_t)fn.n_pass * fn.pass_w - (int64_t)l2.Kp * l2.Np;
-    }
-    // activation scratch: ping-pong buffers [chunk][maxKp]; with the fused kernel in front and the tail kernel behind
-    // only ONE of them is ever used (h2), and the raw output never leaves the SM
-    c->act_elems = (size_t)chunk * (size_t)maxKp;
-    const bool one_buffer = fused && tail && n_layers == 4;
-    for (int b = 0; b < (one_buffer ? 1 : 2); ++b) {
-        CU_TRY(c, cudaMalloc(&c->act[b], c->act_elems * sizeof(__nv_bfloat16)), "cudaMalloc(activations)");
-        CU_TRY(c, cudaMemset(c->act[b], 0, c->act_elems * sizeof(__nv_bfloat16)), "cudaMemset(activations)");
-    }
-    if (!tail) {
-        CU_TRY(c, cudaMalloc(&c->o_buf, (size_t)n_species * chunk * sizeof(float)), "cudaMalloc(o_buf)");
-        CU_TRY(c, cudaMemset(c->o_buf, 0, (size_t)n_species * chunk * sizeof(float)), "cudaMemset(o_buf)");
-    }
-    for (int l = fused ? 2 : 0; l < n_layers; ++l) {
-        LayerBf16 &ly = c->lay[l];
-        std::string terr;
-        if (!encode_tmap_bf16(&ly.tmapA, c->act[l & 1], (uint64_t)ly.Kp, (uint64_t)chunk, (uint64_t)ly.Kp * 2, 128, &terr))
-            return fail(c, GPUANN_ERR_CUDA, "gpuann_load_net: " + terr);
-    }
-    if (tail) {
-        TailNet &tn = c->tail;
-        const LayerBf16 &l3 = c->lay[n_layers - 2], &l4 = c->lay[n_layers - 1];
-        TailArgs &ta = tn.args;
-        ta.Ns = n_species;
-        ta.Np = l4.Np;
-        ta.K3p = l3.Kp;
-        ta.H3p = l3.Np;
-        tail_plan(l3.Np, &ta.n0, &ta.n1);
-        ta.bias3 = l3.bias;
-        ta.newton_max_iter = po.newton_max_iter;
-        ta.inv_lambda_int = po.inv_lambda_int;
-        ta.lambda_zero = po.lambda_zero;
-        ta.lambda = pre.lambda;
-        ta.inv_lambda = pre.inv_lambda;
-        ta.newton_tol = po.newton_tol;
-        ta.T_min = po.T_min;
-        ta.T_max = po.T_max;
-        for (int k = 0; k < kTailMaxNs; ++k) ta.b4[k] = k < n_species ? biases[n_layers - 1][k] : 0.f;
-        std::string terr;
-        if (!encode_tmap_bf16(&tn.tmapW3a, l3.W, (uint64_t)l3.Kp, (uint64_t)l3.Np, (uint64_t)l3.Kp * 2, (uint32_t)(ta.n0 / 2), &terr) ||
-            !encode_tmap_bf16(&tn.tmapW3b, l3.W, (uint64_t)l3.Kp, (uint64_t)l3.Np, (uint64_t)l3.Kp * 2,
-                              (uint32_t)(ta.n1 > 0 ? ta.n1 / 2 : 8), &terr) ||
-            !encode_tmap_bf16(&tn.tmapW4, l4.W, (uint64_t)l4.Kp, (uint64_t)l4.Np, (uint64_t)l4.Kp * 2, (uint32_t)(l4.Np / 2), &terr))
-            return fail(c, GPUANN_ERR_CUDA, "gpuann_load_net: " + terr);
-        // fused kernel directly in front: h2 travels in the blocked layout (common.cuh, FusedNet)
-        ta.a_blocked = one_buffer ? 1 : 0;
-        c->fused.h2_blocked = one_buffer;
-        if (one_buffer && !encode_tmap_bf16_linear(&tn.tmapAb, c->act[0], (uint64_t)chunk * (uint64_t)l3.Kp, &terr))
-            return fail(c, GPUANN_ERR_CUDA, "gpuann_load_net: " + terr);
-        tn.on = true;
-    }
-    c->issued_mac_per_cell = mac;
+    const bool fused = c->net0.fused.on, tail = c->net0.tail.on;
     c->variant = f16 ? "fp16-fused+tail"
                      : (fused ? (tail ? "bf16-fused+tail" : "bf16-fused") : (tail ? "bf16-layerwise+tail" : "bf16-layerwise"));
+    c->net_loaded = true;
+    return GPUANN_OK;
+}
+
+int gpuann_load_net_ensemble(gpuann_ctx *c, int n_species, int n_layers, const int *sizes, const float *const *weights,
+                             const float *const *biases, const float *in_mean, const float *in_std, const float *out_mean,
+                             const float *out_std, double lambda) {
+    if (!c) return fail(nullptr, GPUANN_ERR_INVALID_ARG, "gpuann_load_net_ensemble: ctx is NULL");
+    {
+        const int rc0 = load_prologue(c, "gpuann_load_net_ensemble", n_species, n_layers, sizes, 1, n_species, weights, biases,
+                                      in_mean, in_std, out_mean, out_std, lambda);
+        if (rc0 != GPUANN_OK) return rc0;
+    }
+    if (c->prm.precision == GPUANN_PRECISION_FP32)
+        return fail(c, GPUANN_ERR_UNSUPPORTED, "gpuann_load_net_ensemble: tensor path only (BF16 or FP16 context)");
+    DeviceGuard g(c->device);
+    int rc = plan_and_alloc(c, n_species, n_layers, sizes, true);
+    if (rc != GPUANN_OK) return rc;
+    c->ens.resize((size_t)n_species);
+    int64_t mac_total = 0;
+    for (int k = 0; k < n_species; ++k) {
+        int64_t mac = 0;
+        rc = build_subnet(c, c->ens[(size_t)k], 1, n_layers, sizes, weights + (size_t)k * n_layers, biases + (size_t)k * n_layers, &mac);
+        if (rc != GPUANN_OK) return rc;
+        mac_total += mac;
+        if (!(c->ens[(size_t)k].fused.on && c->ens[(size_t)k].tail.on && n_layers == 4))
+            return fail(c, GPUANN_ERR_UNSUPPORTED,
+                        "gpuann_load_net_ensemble: every net must run the fused + tail kernels (4 weight matrices, first hidden layer >= 128, last <= 416)");
+    }
+    c->cur = &c->ens[0];
+    c->issued_mac_per_cell = mac_total;
+    c->variant = c->prm.precision == GPUANN_PRECISION_FP16 ? "fp16-ensemble" : "bf16-ensemble";
     c->net_loaded = true;
     return GPUANN_OK;
 }
@@ -448,7 +539,7 @@ int gpuann_load_thermo(gpuann_ctx *c, int n_species, const double *nasa_lo, cons
         h->inv_W[k] = 1.0 / W[k];
     }
     {
-        TailArgs &ta = c->tail.args;  // the tail kernel takes the table by value (first kTailMaxNs species)
+        TailArgs &ta = c->net0.tail.args;  // the tail kernel takes the table by value (first kTailMaxNs species)
         ta.two_ranges = h->two_ranges;
         std::memset(&ta.th, 0, sizeof(ta.th));  // species beyond Ns of the kernel's padded range: all-zero constants
         for (int k = 0; k < kTailMaxNs && k < n_species; ++k) {
@@ -511,23 +602,38 @@ struct ChunkOut {
 // the tensor path for the chunk [c0, c0+cn): z -> layers -> (raw output | update S4-S8)
 int run_chunk_bf16(Ctx *c, int64_t n, int64_t c0, int64_t cn, const float *T, const float *p, const float *Y, bool use_idx,
                    const ChunkOut &out, cudaStream_t s) {
+    if (!c->ens.empty()) {
+        // per-species ensemble (R24): net k's forward pass (fused kernel + tail kernel in its
+        // forward-only mode) writes row k of the raw output; S4-S8 then run in the stand-alone update kernel
+        const bool raw_e = out.o_raw != nullptr;
+        float *o = raw_e ? out.o_raw : c->o_buf;
+        const int64_t stride = raw_e ? out.o_stride : c->chunk;
+        for (size_t k = 0; k < c->ens.size(); ++k) {
+            c->cur = &c->ens[k];
+            CU_TRY(c, launch_fused_l1l2(c, n, c0, cn, T, p, Y, use_idx, s), "fused kernel");
+            CU_TRY(c, launch_tail(c, n, c0, cn, nullptr, p, nullptr, nullptr, 1.0, o + (int64_t)k * stride, stride, use_idx, ExtraOut{}, s),
+                   "tail kernel");
+        }
+        if (!raw_e) CU_TRY(c, launch_post(c, n, c0, cn, out.T, out.Y, out.h, c->o_buf, c->chunk, out.dt, use_idx, s), "update kernel");
+        return GPUANN_OK;
+    }
     int l0 = 0;
-    if (c->fused.on) {
+    if (c->cur->fused.on) {
         CU_TRY(c, launch_fused_l1l2(c, n, c0, cn, T, p, Y, use_idx, s), "fused kernel");
         l0 = 2;
     } else {
-        CU_TRY(c, launch_pre_bf16(c, n, c0, cn, T, p, Y, use_idx, c->act[0], c->lay[0].Kp, s), "pre kernel");
+        CU_TRY(c, launch_pre_bf16(c, n, c0, cn, T, p, Y, use_idx, c->act[0], c->cur->lay[0].Kp, s), "pre kernel");
     }
     const bool raw = out.o_raw != nullptr;
     for (int l = l0; l < c->L; ++l) {
-        if (c->tail.on && l == c->L - 2) {
+        if (c->cur->tail.on && l == c->L - 2) {
             CU_TRY(c, launch_tail(c, n, c0, cn, out.T, p, out.Y, out.h, out.dt, out.o_raw, out.o_stride, use_idx, out.ex, s), "tail kernel");
             return GPUANN_OK;
         }
         const bool last = l == c->L - 1;
         __nv_bfloat16 *nxt = last ? nullptr : c->act[(l + 1) & 1];
         CU_TRY(c,
-               launch_layer_bf16(c, l, cn, &c->lay[l].tmapA, nxt, last ? 0 : c->lay[l + 1].Kp,
+               launch_layer_bf16(c, l, cn, &c->cur->lay[l].tmapA, nxt, last ? 0 : c->cur->lay[l + 1].Kp,
                                  last ? (raw ? out.o_raw : c->o_buf) : nullptr, raw ? out.o_stride : c->chunk, c0, use_idx, s),
                "layer kernel");
     }
@@ -569,7 +675,7 @@ int gpuann_chem_step_ex(gpuann_ctx *c, int64_t n, float *T, const float *p, floa
         ex.rho = xo->rho;
         ex.psi = xo->psi;
     }
-    if (ex.any() && c->prm.precision != GPUANN_PRECISION_FP32 && !c->tail.on)
+    if (ex.any() && c->prm.precision != GPUANN_PRECISION_FP32 && (!c->net0.tail.on || !c->ens.empty()))
         return fail(c, GPUANN_ERR_UNSUPPORTED, "gpuann_chem_step_ex: the extra outputs need the tail kernel (Ns <= 48, last hidden layer <= 416)");
     DeviceGuard g(c->device);
     cudaStream_t s = reinterpret_cast<cudaStream_t>(stream);

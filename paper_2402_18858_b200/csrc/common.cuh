@@ -140,6 +140,15 @@ struct TailNet {
     TailArgs args{};
 };
 
+// One network of the tensor path: its layers, the fused-kernel and tail-kernel set-up.  A context holds ONE (the net of
+// gpuann_load_net) or Ns (the per-species ensemble of gpuann_load_net_ensemble, each with a single output).
+struct SubNet {
+    int n_out = 0;                 // outputs of this net: Ns, or 1 in an ensemble
+    LayerBf16 lay[kMaxLayers]{};
+    FusedNet fused;
+    TailNet tail;
+};
+
 struct Ctx {
     gpuann_params prm{};
     int device = 0;
@@ -159,15 +168,15 @@ struct Ctx {
     size_t w32_count = 0, b32_count = 0;
     int max_width = 0;
     // BF16 path
-    LayerBf16 lay[kMaxLayers]{};
+    SubNet net0;                              // gpuann_load_net
+    std::vector<SubNet> ens;                  // gpuann_load_net_ensemble: net k yields o_k (R24)
+    SubNet *cur = &net0;                      // the net the launchers below read (set before every launch)
     int64_t chunk = 0;                        // cells per pass
     __nv_bfloat16 *act[2] = {nullptr, nullptr};  // ping-pong activation buffers [chunk][maxKp]
     size_t act_elems = 0;
     float *o_buf = nullptr;                   // [Ns][chunk] raw output of the chunk
     int64_t issued_mac_per_cell = 0;
     const char *variant = "none";
-    FusedNet fused;
-    TailNet tail;
 
     // thermo
     bool thermo_loaded = false;

@@ -517,7 +517,7 @@ void fused_plan(int H2p, int *n_pass, int *pass_w, int *n0, int *n1) {
 cudaError_t launch_fused_l1l2(Ctx *c, int64_t n, int64_t c0, int64_t cn, const float *T, const float *p, const float *Y,
                               bool use_idx, cudaStream_t s) {
     if (cn <= 0) return cudaSuccess;
-    const FusedNet &fn = c->fused;
+    const FusedNet &fn = c->cur->fused;
     FusedArgs fa{};
     fa.n = n;
     fa.c0 = c0;
@@ -530,12 +530,12 @@ cudaError_t launch_fused_l1l2(Ctx *c, int64_t n, int64_t c0, int64_t cn, const f
     fa.D = c->sizes[0];
     fa.Kz = (c->sizes[0] + 2 + 15) / 16;
     fa.H1p = (c->sizes[1] + kFK - 1) / kFK * kFK;
-    fa.H2p = c->lay[1].Np;
+    fa.H2p = c->cur->lay[1].Np;
     fa.n_pass = fn.n_pass;
     fa.pass_w = fn.pass_w;
     fa.n0 = fn.n0;
     fa.n1 = fn.n1;
-    fa.bias2 = c->lay[1].bias;
+    fa.bias2 = c->cur->lay[1].bias;
     fa.h2 = c->act[0];
     fa.h2_blocked = fn.h2_blocked ? 1 : 0;
     fa.f16 = c->prm.precision == GPUANN_PRECISION_FP16 ? 1 : 0;

@@ -323,7 +323,7 @@ cudaError_t launch_layer_bf16(Ctx *c, int layer, int64_t rows, const CUtensorMap
                               int out_ld, float *out_f32, int64_t out_f32_stride, int64_t c0, bool use_count,
                               cudaStream_t s) {
     if (rows <= 0) return cudaSuccess;
-    const LayerBf16 &ly = c->lay[layer];
+    const LayerBf16 &ly = c->cur->lay[layer];
     GemmArgs ga{};
     ga.Kp = ly.Kp;
     ga.Np = ly.Np;

@@ -611,9 +611,9 @@ void tail_plan(int H3p, int *n0, int *n1) {
 cudaError_t launch_tail(Ctx *c, int64_t n, int64_t c0, int64_t cn, float *T, const float *p, float *Y, const float *h,
                         double dt, float *o_raw, int64_t o_stride, bool use_idx, const ExtraOut &ex, cudaStream_t s) {
     if (cn <= 0) return cudaSuccess;
-    TailNet &tn = c->tail;
+    TailNet &tn = c->cur->tail;
     TailArgs &ta = tn.args;  // the constant part (thermo, net parameters) was filled at load time
-    const LayerBf16 &l3 = c->lay[c->L - 2], &l4 = c->lay[c->L - 1];
+    const LayerBf16 &l3 = c->cur->lay[c->L - 2], &l4 = c->cur->lay[c->L - 1];
     ta.n = n;
     ta.c0 = c0;
     ta.rows = cn;
@@ -629,7 +629,7 @@ cudaError_t launch_tail(Ctx *c, int64_t n, int64_t c0, int64_t cn, float *T, con
     ta.o_raw = o_raw;
     ta.o_stride = o_stride;
     ta.counters = c->counters;
-    for (int k = 0; k < c->Ns; ++k) {
+    for (int k = 0; k < ta.Ns; ++k) {
         ta.sA[k] = (float)(dt * (double)c->post.out_std[k]);
         ta.sC[k] = (float)(dt * ((double)c->post.out_std[k] * (double)ta.b4[k] + (double)c->post.out_mean[k]));
     }
@@ -651,9 +651,9 @@ cudaError_t launch_tail(Ctx *c, int64_t n, int64_t c0, int64_t cn, float *T, con
     cfg.numAttrs = 1;
     (void)l4;
     // species beyond Ns of the padded range must carry all-zero constants (the kernel's arithmetic is unguarded)
-    for (int k = c->Ns; k < kTailMaxNs; ++k) ta.sA[k] = ta.sC[k] = 0.f;
+    for (int k = ta.Ns; k < kTailMaxNs; ++k) ta.sA[k] = ta.sC[k] = 0.f;
     const bool fast = !ta.lambda_zero && ta.inv_lambda_int == 10 && !ta.two_ranges;
-    return cudaLaunchKernelEx(&cfg, tail_kernel(c->Ns, fast), ta.a_blocked ? tn.tmapAb : l3.tmapA, tn.tmapW3a, tn.tmapW3b, tn.tmapW4, ta);
+    return cudaLaunchKernelEx(&cfg, tail_kernel(ta.Ns, fast), ta.a_blocked ? tn.tmapAb : l3.tmapA, tn.tmapW3a, tn.tmapW3b, tn.tmapW4, ta);
 }
 
 }  // namespace gpuann

@@ -192,3 +192,13 @@ def make_problem(cfg: Config, n: Optional[int] = None, seed: Optional[int] = Non
     out_mean = np.zeros(Ns, dtype=np.float32)
     out_std = np.full(Ns, cfg.sigma_out, dtype=np.float32)
     return Problem(cfg, n, state, thermo, net, out_mean, out_std)
+
+
+def gen_ensemble(cfg: Config, seed: int):
+    """SURVEY.md 8(f) NEXT-1 / PAPER.md:103: Ns nets of the shape `D - hidden... - 1` drawn like G3 (Xavier-uniform weights,
+    U[+-1/sqrt(fan_in)] biases, net after net from one generator), rounded like the config's single net.  Returns
+    (sizes, weights[k][l], biases[k][l])."""
+    rng = np.random.default_rng(seed)
+    sizes = (2 + cfg.n_species,) + tuple(cfg.hidden) + (1,)
+    nets = [gen_net(rng, sizes, bf16_weights=(cfg.precision == 1), f16_weights=(cfg.precision == 2)) for _ in range(cfg.n_species)]
+    return sizes, [n.weights for n in nets], [n.biases for n in nets]

@@ -427,3 +427,37 @@ def test_fp16_unsupported_shapes_fail_loudly():
         assert e.value.status == 3
     finally:
         B.gpuann_destroy(ctx)
+
+
+# ------------------------------------------------------------------ per-species ensemble (R24)
+@pytest.mark.parametrize("name,n", [("c2", 128 * 6 + 19), ("c1", 128 * 20 + 3), ("c4", 128 * 8 + 77)])
+def test_ensemble_of_one_output_nets(name, n):
+    """Ns nets D-H1-H2-H3-1 through gpuann_load_net_ensemble against the oracle's O3' (n_nets = Ns): every BF16-path gate."""
+    import dataclasses
+    cfg = I.get_config(name)
+    pr = G.prepare(cfg, n=n, seed=31)
+    sizes, ws, bs = I.gen_ensemble(cfg, seed=99)
+    prm = B.gpuann_default_params()
+    prm.precision = cfg.precision
+    prm.newton_max_iter, prm.newton_tol = pr.model.newton_max_iter, pr.model.newton_tol
+    prm.T_min, prm.T_max, prm.T_active = pr.model.T_min, pr.model.T_max, pr.model.T_active
+    ctx = B.gpuann_create(prm)
+    try:
+        B.gpuann_load_net_ensemble(ctx, cfg.n_species, sizes, ws, bs, pr.in_mean, pr.in_std, pr.prob.out_mean,
+                                   pr.prob.out_std, cfg.lam)
+        th = pr.prob.thermo
+        B.gpuann_load_thermo(ctx, cfg.n_species, th.nasa_lo, th.nasa_hi, th.T_mid, th.W)
+        _, variant = B.gpuann_describe(ctx)
+        assert variant == "bf16-ensemble"
+        g = G.run_gpu(ctx, pr)
+        me = dataclasses.replace(pr.model, sizes=sizes, weights=ws, biases=bs, ensemble=True)
+        st = pr.prob.state
+        ref = oracle.Oracle(me).chem_step(st.T, st.p, st.Y, pr.h, cfg.dt)
+        raw_ref = oracle.Oracle(dataclasses.replace(me, T_active=0.0)).chem_step(st.T, st.p, st.Y, pr.h, cfg.dt)
+        act = ref.flags != 4
+        w = G.check_all_bf16(g, ref, mask=act, raw_ref=raw_ref)
+        assert np.array_equal(g.T_new[~act], st.T[~act]) and np.array_equal(g.Y_new[:, ~act], st.Y[:, ~act])
+        assert g.stats[0] == int(act.sum()) and g.stats[1] == int((ref.flags[act] & 1).sum())
+        print(f"{name} ensemble: {w}")
+    finally:
+        B.gpuann_destroy(ctx)

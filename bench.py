@@ -242,8 +242,16 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     B.gpuann_load_thermo(ctx, Ns, th.nasa_lo, th.nasa_hi, th.T_mid, th.W)
     B.gpuann_enthalpy(ctx, n, T0.data_ptr(), Y0.data_ptr(), h_d.data_ptr(), stream)
     mean, std = B.gpuann_input_moments(ctx, n, Ns, T0.data_ptr(), p_d.data_ptr(), Y0.data_ptr(), cfg.lam, stream)
-    B.gpuann_load_net(ctx, Ns, prob.net.sizes, prob.net.weights, prob.net.biases, mean.astype(np.float32),
-                      std.astype(np.float32), prob.out_mean, prob.out_std, cfg.lam)
+    flop_per_cell = float(cfg.flop_per_cell)
+    if args.ensemble:   # the paper's per-species architecture: Ns nets D-H1-H2-H3-1
+        e_sizes, e_w, e_b = I.gen_ensemble(cfg, seed=cfg.index + 7000)
+        B.gpuann_load_net_ensemble(ctx, Ns, e_sizes, e_w, e_b, mean.astype(np.float32), std.astype(np.float32),
+                                   prob.out_mean, prob.out_std, cfg.lam)
+        flop_per_cell = 2.0 * Ns * sum(e_sizes[i] * e_sizes[i + 1] for i in range(len(e_sizes) - 1))
+        del e_w, e_b
+    else:
+        B.gpuann_load_net(ctx, Ns, prob.net.sizes, prob.net.weights, prob.net.biases, mean.astype(np.float32),
+                          std.astype(np.float32), prob.out_mean, prob.out_std, cfg.lam)
     T_d, Y_d = T0.clone(), Y0.clone()
 
     def restore():
@@ -317,9 +325,9 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         flop_step = 2.0 * sizes[l] * sizes[l + 1] * n_act_per_step
     elif dom_name == "bf16_fused":
         # the fused kernel holds layers 1 and 2 only (algorithmic: the per-pass recompute of layer 1 is not counted)
-        flop_step = 2.0 * (sizes[0] * sizes[1] + sizes[1] * sizes[2]) * n_act_per_step
+        flop_step = 2.0 * (sizes[0] * sizes[1] + sizes[1] * sizes[2]) * n_act_per_step * (Ns if args.ensemble else 1)
     else:
-        flop_step = float(cfg.flop_per_cell) * n_act_per_step
+        flop_step = flop_per_cell * n_act_per_step
     dom_ms_per_step = dom_ms / args.steps
     achieved = flop_step / (dom_ms_per_step * 1e-3) / 1e12
     # DRAM bytes of the dominant kernel per launch: dram__bytes_read.sum + dram__bytes_write.sum of the committed
@@ -340,7 +348,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         "flop_per_step_algorithmic": flop_step,
         "kernel_classes_ms_per_step": {k: v[0] / args.steps for k, v in classes.items()},
     }
-    whole_tflops = cfg.flop_per_cell * (n_act_per_step * world) / ((ms_total / args.steps) * 1e-3) / 1e12
+    whole_tflops = flop_per_cell * (n_act_per_step * world) / ((ms_total / args.steps) * 1e-3) / 1e12
     roofline["whole_step"] = {
         "achieved": whole_tflops,
         "frac_of_measured_burst": whole_tflops / peaks["bf16_tflops"],
@@ -401,7 +409,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         ms_s = np.array([e0.elapsed_time(e1) for e0, e1 in evs])
         tail_half = ms_s[len(ms_s) // 2:]
         ms_sust, _ = aggregate_over_ranks(float(np.median(tail_half)), 0, dist if world > 1 else None, dev)
-        tf_s = cfg.flop_per_cell * (n_act_per_step * world) / (ms_sust * 1e-3) / 1e12
+        tf_s = flop_per_cell * (n_act_per_step * world) / (ms_sust * 1e-3) / 1e12
         sustained = {"seconds": args.sustain, "steps": int(len(ms_s)), "ms_per_step_median_second_half": ms_sust,
                      "ms_per_step_first_20_median": float(np.median(ms_s[:20])), "cells_per_s": n * world / (ms_sust * 1e-3),
                      "tflops": tf_s, "frac_of_measured_burst": tf_s / peaks["bf16_tflops"],
@@ -411,7 +419,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     B.gpuann_destroy(ctx)
 
     cpu_baseline = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+    if rank == 0 and world == 1 and not args.no_cpu_baseline and not args.ensemble:
         sample = calibrated_sample(cfg, prob, target_s=15.0)
         v, threads, secs, s = oracle_sample_run(cfg, prob, sample)
         import oracle
@@ -428,7 +436,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
             "warmup": max(args.warmup, 3), "ms_per_step": ms_total / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": {0: "f32", 1: "bf16", 2: "f16"}[cfg.precision],
             "data": "synthetic",
-            "config": {"workload": workload_name(cfg, n), "cells_per_gpu": n, "variant": variant + ("+ex(rr,hrr,cp,rho,psi)" if args.ex else ""),
+            "config": {"workload": workload_name(cfg, n) + (f", per-species ensemble of {Ns} nets (PAPER.md:103)" if args.ensemble else ""), "cells_per_gpu": n, "variant": variant + ("+ex(rr,hrr,cp,rho,psi)" if args.ex else ""),
                        "l2": "state (184 B/cell x n) larger than L2 and restored from a pristine copy between steps",
                        "parallelism": f"cells sharded over {world} GPU(s), no collective on the data path"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
@@ -454,6 +462,8 @@ def main():
     ap.add_argument("--cells", type=int, default=0, help="override the cell count of the config (per GPU)")
     ap.add_argument("--chunk", type=int, default=0, help="override the library's cells-per-pass")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ensemble", action="store_true",
+                    help="the per-species ensemble of the paper (Ns nets with one output each) instead of the single net")
     ap.add_argument("--ex", action="store_true", help="time gpuann_chem_step_ex with every optional output requested")
     ap.add_argument("--sustain", type=float, default=0.0,
                     help="also run the step back to back for this many seconds and report the sustained figure")

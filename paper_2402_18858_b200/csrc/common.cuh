@@ -91,7 +91,7 @@ struct FusedNet {
     //     h2b[tile][kp = column / 8][row 0..127][8 columns]   (16-byte pieces; a (tile, kp) slab is 2 KB)
     // so that (a) a drain warp's store instruction -- lane = row, one 16-byte piece -- writes 512 contiguous bytes instead
     // of 32 pieces 1600 bytes apart (the row-major stores cost 6,400 LSU line transactions per pass and made the drain
-    // 10 k clk long; profiles/r02_fused.md), and (b) a [128 x 64] A stage of the tail kernel is ONE contiguous 16 KB
+    // 10 k clk long), and (b) a [128 x 64] A stage of the tail kernel is ONE contiguous 16 KB
     // piece of global memory, read by the MMA through a no-swizzle descriptor (LBO 2048, SBO 128).
     bool h2_blocked = false;
 };

@@ -4,16 +4,18 @@
 //     h2 = GELU(h1 W2^T + b2)    [128 x H2]   -> global scratch, BF16 (input of the tail kernel)
 // Why: layer 2 holds 78 % of the FLOPs and its A operand h1 (3.2 KB/cell) is the largest activation.
 // TMEM (512 columns) cannot hold a 128 x 800 FP32 accumulator, so the H2 columns are processed in n_pass passes of
-// <= 416 columns and h1 is recomputed per pass (4 % more MMA work; the alternatives -- h1 through L2 or through
-// distributed shared memory -- cost more bandwidth than either has, profiles/r02_fused.md).
+// <= 400 columns and h1 is recomputed per pass (4 % more MMA work; the alternatives -- h1 through L2 or through
+// distributed shared memory -- cost more bandwidth than either has).
 //
-// Data path of one 32-column piece of h1 ("slot step"; three TMEM slots of 32 columns):
-//     tcgen05.mma  L1acc[slot] (128 x 32 FP32, TMEM) = z tile (smem) x W1 rows (smem); b1 rides in two extra K columns
-//     workers      tcgen05.ld -> 2 GELU -> BF16 pairs -> tcgen05.st into the SAME slot (16 columns)
-//     tcgen05.mma  acc[0..pass_w) += h1 piece (A operand read from TENSOR MEMORY) x W2 k-slab (smem)
+// Data path of one 32-column piece of h1 ("slot step"; TMEM columns 400..511: two layer-1 accumulators of 32 FP32 columns
+// and three A slots of 16 columns):
+//     tcgen05.mma  L1acc[g & 1] (128 x 32 FP32, TMEM) = z tile (smem) x W1 rows (smem); b1 rides in two extra K columns
+//     workers      tcgen05.ld (accumulator free again) -> 2 GELU -> BF16 pairs -> tcgen05.st into A slot g % 3
+//     tcgen05.mma  acc[0..pass_w) += A slot (A operand read from TENSOR MEMORY) x W2 k-slab (smem)
 // so h1 costs no shared-memory bandwidth at all: the only shared-memory streams left are the W2 / W1 slabs written by
 // TMA and read by the MMAs (the first version of this kernel kept h1 in a shared-memory ring and ran the MMAs' operand
 // reads + TMA writes + the producers' stores at ~120 % of the 128 B/clk the shared memory delivers at full tensor rate).
+// Five pieces are in flight (two accumulators + three slots), so neither issuer waits for a conversion in steady state.
 //
 // CTA PAIRS: clusters of 2 whose even CTA (the leader) issues every tcgen05.mma with cta_group::2 -- M = 256 = the
 // 128-cell tiles of both CTAs, B read half from each CTA's shared memory: a CTA stages and reads HALF of every W1 / W2
@@ -22,15 +24,14 @@
 // Roles (512 threads, one CTA per SM, tiles of 128 cells walked with stride gridDim.x):
 //   warp 14     TMA (both CTAs): own half of each W2 k-slab [pass_w/2 x 64] (ring of 6) and of each W1 row block (ring
 //               of 4); completion is counted on the LEADER's full barriers
-//   warp 15     (leader) layer-2 issuer: acc += slot (TMEM) x W2 slab; tells the layer-1 issuer that the slot's MMAs are QUEUED
-//   warp 13     (leader) layer-1 issuer: layer 1 of step g + 3 goes INTO THE SLOT step g's layer-2 MMAs read, as soon as
-//               those are queued, not completed -- the tensor pipe executes in issue order -- so the workers have two
-//               full steps (~1000 clk) to convert a slot before its layer-2 MMAs are issued.  Two issuer warps because
-//               ONE warp's instruction stream (waits ~90 clk each, descriptor set-up, 6 MMAs, 2-3 commits) took ~1000 clk
-//               per step against the 480 clk the tensor pipe needs (profiles/r02_fused.md)
+//   warp 15     (leader) layer-2 issuer: acc += A slot (TMEM) x W2 slab; its commit hands the slot back to the workers
+//   warp 13     (leader) layer-1 issuer: runs up to two accumulators ahead of the workers.  Two issuer warps because ONE
+//               warp's instruction stream (waits ~90 clk each, descriptor set-up, 6 MMAs, 2-3 commits) took ~1000 clk
+//               per step against the 480 clk the tensor pipe needs (profiles/r02_ncu_full_c2.md)
 //   warp 12     z builder: state (SoA, 128-bit loads; gathered through idx under compaction) -> Box-Cox -> z-score ->
 //               BF16 -> 128-byte-swizzled smem tile, double buffered across tiles
-//   warps 0-11  workers, three groups of four warps (one per TMEM lane quarter); group s owns slot s.  At the end of
+//   warps 0-11  workers, three groups of four warps (one per TMEM lane quarter); group s converts steps g = s mod 3 into A
+//               slot s.  At the end of
 //               a pass ALL twelve drain the accumulator (tcgen05.ld -> + b2 -> 2 GELU -> BF16 -> h2), every third
 //               32-column block each: the drain is bound by the SFU (one tanh per element), so it takes all four SM
 //               sub-partitions to keep the tensor pipe's idle time per pass near 51,200 / 14 per clk = 3.7 k clk
@@ -47,14 +48,16 @@ constexpr int kFK = 64;          // K elements per shared-memory row (128 B) = h
 constexpr int kSub = 32;         // h1 columns per slot step
 constexpr int kW2Stages = 6;
 constexpr int kW1Stages = 4;
-constexpr int kL1Slots = 3;
-constexpr int kAccCols = 416;    // TMEM columns of the layer-2 accumulator (max pass width)
-constexpr int kL1Col = kAccCols; // the three slots live in columns 416..511
+constexpr int kL1Accs = 2;       // layer-1 accumulators (32 FP32 columns each)
+constexpr int kASlots = 3;       // converted h1 pieces = A operands of layer 2 (16 columns of BF16 pairs each)
+constexpr int kAccCols = 400;    // TMEM columns of the layer-2 accumulator (max pass width)
+constexpr int kL1Col = kAccCols;                   // 400..463: the two layer-1 accumulators
+constexpr int kACol = kL1Col + kL1Accs * kSub;     // 464..511: the three A slots
 constexpr int kFusedThreads = 512;
 constexpr int kWorkerGroups = 3;
 // Warp numbering follows the issue arbiter, which serves the HIGHEST warp id of a sub-partition first (measured: as warp 1,
 // behind three GELU-dense worker warps on its sub-partition, the MMA issuer got an issue slot every ~10 clk and needed
-// 1000 clk per slot step; profiles/r02_fused.md): workers are warps 0..11, the latency-critical single-thread roles sit on
+// 1000 clk per slot step): workers are warps 0..11, the latency-critical single-thread roles sit on
 // top, one per sub-partition.
 constexpr int kWarpZ = 12;
 constexpr int kWarpMma1 = 13;  // layer-1 issuer
@@ -76,7 +79,8 @@ constexpr size_t kFusedSmem = 1024 + kOffBar + 512;
 // barrier indices
 enum {
     bW2Full = 0, bW2Empty = bW2Full + kW2Stages, bW1Full = bW2Empty + kW2Stages, bW1Empty = bW1Full + kW1Stages,
-    bL1Full = bW1Empty + kW1Stages, bAFull = bL1Full + kL1Slots, bSlotFree = bAFull + kL1Slots, bZFull = bSlotFree + kL1Slots, bZEmpty = bZFull + 2,
+    bL1Full = bW1Empty + kW1Stages, bL1Free = bL1Full + kASlots, bAFull = bL1Free + kL1Accs, bAFree = bAFull + kASlots,
+    bZFull = bAFree + kASlots, bZEmpty = bZFull + 2,
     bAccFull = bZEmpty + 2, bAccEmpty = bAccFull + 1, bCount = bAccEmpty + 1
 };
 
@@ -142,11 +146,12 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
     if (threadIdx.x == 0) {
         for (int i = 0; i < kW2Stages; ++i) { ptx::mbar_init(&bars[bW2Full + i], 1); ptx::mbar_init(&bars[bW2Empty + i], 1); }
         for (int i = 0; i < kW1Stages; ++i) { ptx::mbar_init(&bars[bW1Full + i], 1); ptx::mbar_init(&bars[bW1Empty + i], 1); }
-        for (int i = 0; i < kL1Slots; ++i) {
-            ptx::mbar_init(&bars[bL1Full + i], 1);
+        for (int i = 0; i < kASlots; ++i) {
+            ptx::mbar_init(&bars[bL1Full + i], 1);  // one per worker group: "your step's layer-1 accumulator is complete"
             ptx::mbar_init(&bars[bAFull + i], 8);   // the four warps of the slot's group in BOTH CTAs
-            ptx::mbar_init(&bars[bSlotFree + i], 1);
+            ptx::mbar_init(&bars[bAFree + i], 1);
         }
+        for (int i = 0; i < kL1Accs; ++i) ptx::mbar_init(&bars[bL1Free + i], 8);
         for (int i = 0; i < 2; ++i) { ptx::mbar_init(&bars[bZFull + i], 2); ptx::mbar_init(&bars[bZEmpty + i], 1); }
         ptx::mbar_init(&bars[bAccFull], 1);
         ptx::mbar_init(&bars[bAccEmpty], 2 * 4 * kWorkerGroups);
@@ -223,7 +228,7 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
                 ptx::mbar_wait2(&bars[bAFull + slot], (a_ph >> slot) & 1u, &bars[bW2Full + w2.st], w2.ph);
                 ptx::tc_fence_after_sync();
                 a_ph ^= 1u << slot;
-                const uint32_t a_tmem = tmem_base + kL1Col + slot * kSub;
+                const uint32_t a_tmem = tmem_base + kACol + slot * (kSub / 2);
                 const uint64_t db = desc0 + (uint64_t)((kOffW2 + w2.st * kW2StageBytes) >> 4) + (uint64_t)((j & 1) * (kSub * 2 / 16));
                 const bool last_of_pass = j == nsteps - 1;
                 if (ptx::elect_one()) {
@@ -234,16 +239,13 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
                         if (fa.n1 > 0)
                             ptx::umma_bf16_ts_cg2(tmem_base + (uint32_t)fa.n0, a_tmem + 8u * k, db + b1_off + 2 * k, idesc_n1, accum);
                     }
+                    ptx::umma_commit_cg2(&bars[bAFree + slot], 3);  // the slot may be rewritten once these MMAs have read it
                     if (j & 1) ptx::umma_commit_cg2(&bars[bW2Empty + w2.st], 3);
                     if (last_of_pass) ptx::umma_commit_cg2(&bars[bAccFull], 3);
-                    // the slot's layer-2 MMAs are in the tensor pipe's queue: the layer-1 issuer may now queue the MMAs that
-                    // overwrite it (the pipe executes in issue order)
-                    ptx::tc_fence_before_sync();
-                    ptx::mbar_arrive(&bars[bSlotFree + slot]);
                 }
                 __syncwarp();
                 if (j & 1) w2.next(kW2Stages);
-                if (++slot == kL1Slots) slot = 0;
+                if (++slot == kASlots) slot = 0;
                 if (++j == nsteps) {
                     j = 0;
                     acc_ph ^= 1u;
@@ -256,16 +258,16 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
             const uint32_t idesc_l1 = ptx::umma_idesc_bf16_f32(2 * kFM, kSub, F16);
             Ring w1;
             int j1 = 0, pass1 = 0, it1 = 0;
-            uint32_t slot1 = 0, s_ph = 0x7u;  // first use of every slot: nothing to wait for
+            uint32_t grp1 = 0, acc1 = 0, f_ph = 0x3u;  // first use of either accumulator: nothing to wait for
             for (int g = 0; g < total_steps; ++g) {
                 const uint32_t zb = (uint32_t)it1 & 1u;
                 if (j1 == 0 && pass1 == 0) ptx::mbar_wait(&bars[bZFull + zb], ((uint32_t)it1 >> 1) & 1u);
-                ptx::mbar_wait2(&bars[bSlotFree + slot1], (s_ph >> slot1) & 1u, &bars[bW1Full + w1.st], w1.ph);
+                ptx::mbar_wait2(&bars[bL1Free + acc1], (f_ph >> acc1) & 1u, &bars[bW1Full + w1.st], w1.ph);
                 ptx::tc_fence_after_sync();
-                s_ph ^= 1u << slot1;
+                f_ph ^= 1u << acc1;
                 const uint64_t dz = desc0 + (uint64_t)((kOffZ + zb * kZBytes) >> 4);
                 const uint64_t dw = desc0 + (uint64_t)((kOffW1 + w1.st * kW1StageBytes + (uint32_t)(j1 & 1) * kW1SubBytes) >> 4);
-                const uint32_t d_tmem = tmem_base + kL1Col + slot1 * kSub;
+                const uint32_t d_tmem = tmem_base + kL1Col + acc1 * kSub;
                 const bool last_of_tile = pass1 == fa.n_pass - 1 && j1 == nsteps - 1;
                 if (ptx::elect_one()) {
                     if (fa.Kz == 2) {
@@ -274,13 +276,14 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
                     } else {
                         for (int k = 0; k < fa.Kz; ++k) ptx::umma_bf16_ss_cg2(d_tmem, dz + 2 * k, dw + 2 * k, idesc_l1, k ? 1u : 0u);
                     }
-                    ptx::umma_commit_cg2(&bars[bL1Full + slot1], 3);
+                    ptx::umma_commit_cg2(&bars[bL1Full + grp1], 3);
                     if (j1 & 1) ptx::umma_commit_cg2(&bars[bW1Empty + w1.st], 3);
                     if (last_of_tile) ptx::umma_commit_cg2(&bars[bZEmpty + zb], 3);
                 }
                 __syncwarp();
                 if (j1 & 1) w1.next(kW1Stages);
-                if (++slot1 == kL1Slots) slot1 = 0;
+                if (++grp1 == kASlots) grp1 = 0;
+                acc1 ^= 1u;
                 if (++j1 == nsteps) {
                     j1 = 0;
                     if (++pass1 == fa.n_pass) {
@@ -371,8 +374,9 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
         const int grp = warp >> 2;         // slot this group owns; every third 32-column block of the drain
         const int r = q * 32 + lane;             // row of the tile
         const uint32_t lane_addr = tmem_base + ((uint32_t)(q * 32) << 16);
-        const uint32_t slot_addr = lane_addr + kL1Col + (uint32_t)grp * kSub;
+        const uint32_t a_addr = lane_addr + kACol + (uint32_t)grp * (kSub / 2);
         const uint32_t afull = bars_leader + 8u * (bAFull + grp);
+        uint32_t afree_ph = 1u;  // first use of the slot: nothing to wait for
         const int total_passes = my_tiles * fa.n_pass;
         int pass_idx = 0;       // passes drained so far (over all tiles)
         uint32_t l1_ph = 0;
@@ -452,18 +456,25 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
 
         int boundary = nsteps;  // first global step of the next pass
 #pragma unroll 1
-        for (int g = grp; g < total_steps; g += kL1Slots) {
-            // ---- convert this group's slot: L1 accumulator -> 2 GELU -> BF16 pairs, in place (A operand of layer 2)
+        for (int g = grp; g < total_steps; g += kASlots) {
+            // ---- convert this group's step: layer-1 accumulator (g & 1) -> 2 GELU -> BF16 pairs -> A slot `grp`
+            const uint32_t acc = (uint32_t)g & 1u;
             ptx::mbar_wait(&bars[bL1Full + grp], l1_ph);
             l1_ph ^= 1u;
             ptx::tc_fence_after_sync();
             uint32_t v[32];
-            ptx::tmem_ld32(slot_addr, v);
+            ptx::tmem_ld32(lane_addr + kL1Col + acc * kSub, v);
             ptx::tmem_ld_wait();
+            ptx::tc_fence_before_sync();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive_cluster(bars_leader + 8u * (bL1Free + acc));  // the accumulator is in registers
             uint32_t o[16];
 #pragma unroll
             for (int jj = 0; jj < 16; ++jj) o[jj] = ptx::gelu2_pack(__uint_as_float(v[2 * jj]), __uint_as_float(v[2 * jj + 1]), f16);
-            ptx::tmem_st16(slot_addr, o);
+            ptx::mbar_wait(&bars[bAFree + grp], afree_ph);  // the layer-2 MMAs of this slot's previous piece have completed
+            afree_ph ^= 1u;
+            ptx::tc_fence_after_sync();
+            ptx::tmem_st16(a_addr, o);
             ptx::tmem_st_wait();
             ptx::tc_fence_before_sync();
             __syncwarp();

@@ -132,7 +132,7 @@ __device__ __forceinline__ uint32_t mapa_u32(uint32_t local_smem_addr, uint32_t 
 // CUTLASS's ClusterBarrier::arrive: what the arrivals of this library hand over is tensor memory (ordered by tcgen05.wait /
 // tcgen05.fence) or shared memory that only the async proxy reads (ordered by fence.proxy.async), never generic-proxy data
 // of the peer.  The .release.cluster / .acquire.cluster forms cost ~1000 clk per arrive behind outstanding global stores and
-// a CCTL.IVALL (L1 invalidate) per successful wait (profiles/r02_fused.md).
+// a CCTL.IVALL (L1 invalidate) per successful wait.
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
     asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
 }

@@ -29,8 +29,10 @@
  *     as void*; NULL = the legacy default stream).  They never synchronise; calls on one stream are
  *     ordered.  A context must not be used from two streams or two host threads at the same time
  *     (its activation scratch is shared).
- *   - The library allocates device scratch that is bounded by the cell-chunk size (not by n_cells),
- *     plus, when T_active > 0, an int32 index list of n_cells entries (grown lazily).
+ *   - Device scratch: one activation buffer of chunk x H2 BF16 (h2, the only activation that crosses HBM; two buffers of
+ *     chunk x max width on the fallback path), where chunk = min(n_cells rounded up, gpuann_params.chunk_cells) and the
+ *     default chunk is 148 x 128 x 56 = 1,060,864 cells: 1.7 GB for the 23-1600-800-400-21 net -- it grows with n_cells
+ *     up to that chunk, not beyond.  Plus, when T_active > 0, an int32 index list of n_cells entries (grown lazily).
  *   - There is no CPU fallback: without a CUDA device of compute capability 10.x gpuann_create fails
  *     with GPUANN_ERR_UNSUPPORTED.
  */

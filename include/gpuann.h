@@ -30,9 +30,10 @@
  *     ordered.  A context must not be used from two streams or two host threads at the same time
  *     (its activation scratch is shared).
  *   - Device scratch: one activation buffer of chunk x H2 BF16 (h2, the only activation that crosses HBM; two buffers of
- *     chunk x max width on the fallback path), where chunk = min(n_cells rounded up, gpuann_params.chunk_cells) and the
- *     default chunk is 148 x 128 x 56 = 1,060,864 cells: 1.7 GB for the 23-1600-800-400-21 net -- it grows with n_cells
- *     up to that chunk, not beyond.  Plus, when T_active > 0, an int32 index list of n_cells entries (grown lazily).
+ *     chunk x max width on the fallback path), allocated by gpuann_load_net for chunk = gpuann_params.chunk_cells cells
+ *     (default 148 x 128 x 56 = 1,060,864: 1.7 GB for the 23-1600-800-400-21 net; larger fields are processed chunk by
+ *     chunk, so the scratch does not grow with n_cells).  Plus, when T_active > 0, an int32 index list of n_cells
+ *     entries (grown lazily).
  *   - There is no CPU fallback: without a CUDA device of compute capability 10.x gpuann_create fails
  *     with GPUANN_ERR_UNSUPPORTED.
  */

@@ -461,3 +461,33 @@ def test_ensemble_of_one_output_nets(name, n):
         print(f"{name} ensemble: {w}")
     finally:
         B.gpuann_destroy(ctx)
+
+
+# ------------------------------------------------------------------ race detection by repetition (compute-sanitizer is closed on this pool)
+@pytest.mark.parametrize("name,reps", [("c2", 8), ("c4", 3)])
+def test_full_size_runs_are_bit_identical(name, reps):
+    """The bench launch configuration (full field, default chunk, 74 CTA pairs) repeated: every run must reproduce the first
+    bit for bit.  A missing barrier or fence between the issuer, worker and TMA warps of the two tensor kernels shows up
+    here as a few differing cells (the parity tests at full size compare sampled cells only)."""
+    import torch
+    cfg = I.get_config(name)
+    pr = G.prepare(cfg)
+    ctx = G.make_ctx(pr)
+    try:
+        dev = torch.device("cuda:0")
+        st = pr.prob.state
+        T0, p0, Y0, h0 = (torch.from_numpy(np.ascontiguousarray(a)).to(dev) for a in (st.T, st.p, st.Y, pr.h))
+        stream = torch.cuda.current_stream().cuda_stream
+        first = None
+        for r in range(reps):
+            T, Y = T0.clone(), Y0.clone()
+            B.gpuann_chem_step(ctx, cfg.n_cells, T.data_ptr(), p0.data_ptr(), Y.data_ptr(), h0.data_ptr(), cfg.dt, stream)
+            torch.cuda.synchronize()
+            if first is None:
+                first = (T, Y)
+                assert bool(torch.isfinite(T).all()) and bool(torch.isfinite(Y).all())
+            else:
+                assert torch.equal(T.view(torch.int32), first[0].view(torch.int32)), f"run {r}: T differs from run 0"
+                assert torch.equal(Y.view(torch.int32), first[1].view(torch.int32)), f"run {r}: Y differs from run 0"
+    finally:
+        B.gpuann_destroy(ctx)

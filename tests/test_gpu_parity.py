@@ -491,3 +491,48 @@ def test_full_size_runs_are_bit_identical(name, reps):
                 assert torch.equal(Y.view(torch.int32), first[1].view(torch.int32)), f"run {r}: Y differs from run 0"
     finally:
         B.gpuann_destroy(ctx)
+
+
+def test_small_chunks_ex_fp16_and_ensemble():
+    """Several chunks per step (chunk_cells = 512 on 1,157 cells): the optional outputs, the FP16 variant and the ensemble
+    address their per-chunk scratch and their field-sized outputs correctly."""
+    import dataclasses
+    n = 128 * 9 + 5
+    # optional outputs on the FP16 variant, three chunks
+    pr = G.prepare(I.get_config("c2h"), n=n, seed=41)
+    ctx = G.make_ctx(pr, chunk_cells=512)
+    try:
+        g, ex = G.run_gpu_ex(ctx, pr)
+        ref = G.run_oracle(pr)
+        g_raw = G.run_gpu(ctx, pr)
+        G.check_all_fp16(g_raw, ref)
+        assert np.array_equal(g_raw.T_new, g.T_new) and np.array_equal(g_raw.Y_new, g.Y_new)
+        G.check_ex(pr, ref, ex, bf16=True)
+    finally:
+        B.gpuann_destroy(ctx)
+    # ensemble, three chunks, against the one-chunk run of the same context type (bit-identical) and the oracle
+    cfg = I.get_config("c2")
+    pr = G.prepare(cfg, n=n, seed=43)
+    sizes, ws, bs = I.gen_ensemble(cfg, seed=5)
+    res = []
+    for chunk in (512, 0):
+        prm = B.gpuann_default_params()
+        prm.precision, prm.chunk_cells = cfg.precision, chunk
+        ctx = B.gpuann_create(prm)
+        try:
+            B.gpuann_load_net_ensemble(ctx, cfg.n_species, sizes, ws, bs, pr.in_mean, pr.in_std, pr.prob.out_mean,
+                                       pr.prob.out_std, cfg.lam)
+            th = pr.prob.thermo
+            B.gpuann_load_thermo(ctx, cfg.n_species, th.nasa_lo, th.nasa_hi, th.T_mid, th.W)
+            res.append(G.run_gpu(ctx, pr))
+            with pytest.raises(B.GpuannError) as e:      # the optional outputs are not available with an ensemble
+                G.run_gpu_ex(ctx, pr, which=("hrr",))
+            assert e.value.status == 3
+        finally:
+            B.gpuann_destroy(ctx)
+    assert np.array_equal(res[0].T_new, res[1].T_new) and np.array_equal(res[0].Y_new, res[1].Y_new)
+    assert np.array_equal(res[0].o_raw, res[1].o_raw)
+    me = dataclasses.replace(pr.model, sizes=sizes, weights=ws, biases=bs, ensemble=True)
+    st = pr.prob.state
+    ref = oracle.Oracle(me).chem_step(st.T, st.p, st.Y, pr.h, cfg.dt)
+    G.check_all_bf16(res[0], ref)

@@ -393,29 +393,23 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
             int cur_w = fa.H2p - col_base;
             cur_w = cur_w < fa.pass_w ? cur_w : fa.pass_w;
             __nv_bfloat16 *dst_row = fa.h2 + grow * fa.H2p + col_base;
-            const int n_blocks = (cur_w + 31) / 32;
-            const int my_last = ((n_blocks - 1 - grp) / kWorkerGroups) * kWorkerGroups + grp;  // < grp when the group has none
-            if (n_blocks <= grp) {
+            // work split over the three groups: every third full 32-column block, and the 16-column remainder of a pass
+            // (widths are multiples of 16) as two 8-column units for groups 0 and 1 -- 4.25 / 4.25 / 4 blocks at 400 columns
+            const int n_full = cur_w >> 5, rem = cur_w & 31;
+            const bool has_tail = rem > 0 && grp < (rem >> 3);
+            const int my_last = n_full > grp ? ((n_full - 1 - grp) / kWorkerGroups) * kWorkerGroups + grp : -1;
+            if (my_last < 0 && !has_tail) {
                 ptx::tc_fence_before_sync();
                 __syncwarp();
                 if (lane == 0) ptx::mbar_arrive_cluster(bars_leader + 8u * bAccEmpty);
             }
 #pragma unroll 1
-            for (int b = grp; b < n_blocks; b += kWorkerGroups) {
+            for (int b = grp; b < n_full; b += kWorkerGroups) {
                 const int cc = b * 32;
-                const bool full = cc + 32 <= cur_w;  // widths are multiples of 16: the tail piece has 16 columns
                 uint32_t v[32];
-                if (full) ptx::tmem_ld32(lane_addr + (uint32_t)cc, v);
-                else {
-                    uint32_t w[16];
-                    ptx::tmem_ld16(lane_addr + (uint32_t)cc, w);
-#pragma unroll
-                    for (int jj = 0; jj < 16; ++jj) v[jj] = w[jj];
-#pragma unroll
-                    for (int jj = 16; jj < 32; ++jj) v[jj] = 0u;
-                }
+                ptx::tmem_ld32(lane_addr + (uint32_t)cc, v);
                 ptx::tmem_ld_wait();
-                if (b == my_last) {
+                if (b == my_last && !has_tail) {
                     // last accumulator read of this warp: hand the accumulator back to the issuer
                     ptx::tc_fence_before_sync();
                     __syncwarp();
@@ -425,7 +419,7 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
                 uint32_t o[16];
 #pragma unroll
                 for (int jj = 0; jj < 8; ++jj) {
-                    const float4 bb = (full || jj < 4) ? b4[jj] : make_float4(0.f, 0.f, 0.f, 0.f);
+                    const float4 bb = b4[jj];
                     o[2 * jj] = ptx::gelu2_pack(__uint_as_float(v[4 * jj]) + bb.x, __uint_as_float(v[4 * jj + 1]) + bb.y, f16);
                     o[2 * jj + 1] = ptx::gelu2_pack(__uint_as_float(v[4 * jj + 2]) + bb.z, __uint_as_float(v[4 * jj + 3]) + bb.w, f16);
                 }
@@ -436,19 +430,36 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
                         uint4 *dst = reinterpret_cast<uint4 *>(fa.h2) + ((int64_t)tile * (fa.H2p >> 3) + ((col_base + cc) >> 3)) * kFM + r;
                         dst[0] = make_uint4(o[0], o[1], o[2], o[3]);
                         dst[kFM] = make_uint4(o[4], o[5], o[6], o[7]);
-                        if (full) {
-                            dst[2 * kFM] = make_uint4(o[8], o[9], o[10], o[11]);
-                            dst[3 * kFM] = make_uint4(o[12], o[13], o[14], o[15]);
-                        }
+                        dst[2 * kFM] = make_uint4(o[8], o[9], o[10], o[11]);
+                        dst[3 * kFM] = make_uint4(o[12], o[13], o[14], o[15]);
                     }
                 } else if (row_ok) {
                     uint4 *dst = reinterpret_cast<uint4 *>(dst_row + cc);
                     dst[0] = make_uint4(o[0], o[1], o[2], o[3]);
                     dst[1] = make_uint4(o[4], o[5], o[6], o[7]);
-                    if (full) {
-                        dst[2] = make_uint4(o[8], o[9], o[10], o[11]);
-                        dst[3] = make_uint4(o[12], o[13], o[14], o[15]);
-                    }
+                    dst[2] = make_uint4(o[8], o[9], o[10], o[11]);
+                    dst[3] = make_uint4(o[12], o[13], o[14], o[15]);
+                }
+            }
+            if (has_tail) {
+                const int cc = n_full * 32 + grp * 8;
+                uint32_t v[8];
+                ptx::tmem_ld8(lane_addr + (uint32_t)cc, v);
+                ptx::tmem_ld_wait();
+                ptx::tc_fence_before_sync();
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive_cluster(bars_leader + 8u * bAccEmpty);
+                const float4 *b4 = reinterpret_cast<const float4 *>(sBias + col_base + cc);
+                const float4 b0 = b4[0], b1 = b4[1];
+                const uint4 o = make_uint4(ptx::gelu2_pack(__uint_as_float(v[0]) + b0.x, __uint_as_float(v[1]) + b0.y, f16),
+                                           ptx::gelu2_pack(__uint_as_float(v[2]) + b0.z, __uint_as_float(v[3]) + b0.w, f16),
+                                           ptx::gelu2_pack(__uint_as_float(v[4]) + b1.x, __uint_as_float(v[5]) + b1.y, f16),
+                                           ptx::gelu2_pack(__uint_as_float(v[6]) + b1.z, __uint_as_float(v[7]) + b1.w, f16));
+                if (fa.h2_blocked) {
+                    if (tile < n_tiles)
+                        *(reinterpret_cast<uint4 *>(fa.h2) + ((int64_t)tile * (fa.H2p >> 3) + ((col_base + cc) >> 3)) * kFM + r) = o;
+                } else if (row_ok) {
+                    *reinterpret_cast<uint4 *>(dst_row + cc) = o;
                 }
             }
             ++pass_idx;

@@ -536,3 +536,43 @@ def test_small_chunks_ex_fp16_and_ensemble():
     st = pr.prob.state
     ref = oracle.Oracle(me).chem_step(st.T, st.p, st.Y, pr.h, cfg.dt)
     G.check_all_bf16(res[0], ref)
+
+
+def test_full_size_fp16_and_ex_outputs_sampled():
+    """configs[2] at its full size once more, (a) as the FP16 variant and (b) with every optional output requested: oracle
+    parity on first 4,096 + last 4,096 + 16,384 drawn cells, full-field invariants."""
+    # (a)
+    cfg = I.get_config("c2h")
+    pr = G.prepare(cfg)
+    ctx = G.make_ctx(pr)
+    try:
+        g = G.run_gpu(ctx, pr)
+        assert g.stats == (cfg.n_cells, 0, 0)
+        _full_field_invariants(cfg, g)
+        idx = G.sample_indices(cfg.n_cells, np.random.default_rng(77), 16384)
+        ref, sub = G.subset(pr, g, idx)
+        print(f"c2h full: {idx.size} sampled cells, {G.check_all_fp16(sub, ref)}")
+    finally:
+        B.gpuann_destroy(ctx)
+    # (b)
+    cfg = I.get_config("c2")
+    pr = G.prepare(cfg)
+    ctx = G.make_ctx(pr)
+    try:
+        g, ex = G.run_gpu_ex(ctx, pr)
+        idx = G.sample_indices(cfg.n_cells, np.random.default_rng(78), 16384)
+        st = pr.prob.state
+        import dataclasses
+        sub_prob = I.Problem(pr.prob.cfg, int(idx.size), I.State(st.T[idx], st.p[idx], np.ascontiguousarray(st.Y[:, idx])),
+                             pr.prob.thermo, pr.prob.net, pr.prob.out_mean, pr.prob.out_std)
+        sub_pr = dataclasses.replace(pr, prob=sub_prob, h=pr.h[idx])
+        ref = G.run_oracle(sub_pr)
+        sub = G.GpuResult(g.T_new[idx], np.ascontiguousarray(g.Y_new[:, idx]), None, g.stats)
+        G.check_T_bf16(sub, ref)
+        G.check_Y_bf16(sub, ref)
+        ex_sub = {k: (np.ascontiguousarray(v[:, idx]) if v.ndim == 2 else v[idx]) for k, v in ex.items()}
+        print(f"c2 full ex: {G.check_ex(sub_pr, ref, ex_sub, bf16=True)}")
+        for k, v in ex.items():
+            assert np.isfinite(v).all(), k
+    finally:
+        B.gpuann_destroy(ctx)

@@ -62,3 +62,13 @@ def test_two_rank_aggregation_and_sharding():
 def test_single_rank_aggregation_is_identity():
     import bench
     assert bench.aggregate_over_ranks(3.5, 42, None, None) == (3.5, 42)
+
+
+def test_roofline_traffic_comes_from_the_tracked_ncu_table():
+    """bench.py's roofline.traffic is read from profiles/ncu_dram_bytes.csv (ncu --set full captures), never a literal in
+    the code; a configuration without a capture yields None."""
+    import bench
+    t = bench.dram_bytes_from_profiles("bf16_fused", 2, 1048576)
+    assert t is not None and 1.5e9 < t < 2.0e9          # state in + h2 out of the fused kernel at configs[2]
+    assert bench.dram_bytes_from_profiles("bf16_fused", 3, 4194304) is None
+    assert bench.dram_bytes_from_profiles("bf16_tail", 2, 12345) is None

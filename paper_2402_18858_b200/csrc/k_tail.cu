@@ -20,9 +20,11 @@
 //   warps 4-11   drain: tcgen05.ld 32 columns of acc -> + b3 -> 2 GELU -> BF16 -> swizzled 64-column h3 chunk (ring of 2)
 //   warps 12-15  update, one thread per cell: state loads (gathered through idx under compaction) issued BEFORE waiting
 //                for o; species update in FP32 (Y^lambda by lg2/ex2, integer power 1/lambda), sum of Y* and the NASA-7
-//                MIXTURE coefficients sum_k Y_k c_kj accumulated in FP64 while the species stream by, then Newton on the
-//                two mixture polynomials in FP64: 11 FMAs per iteration instead of 11 Ns (one-range tables; a two-range
-//                table re-selects per species and iteration).  DESIGN.md "Precision of the scalar math".
+//                MIXTURE coefficients sum_k Y_k c_kj accumulated while the species stream by (FP32 in the FAST instance,
+//                FP64 in the generic one), then Newton on the two mixture polynomials in FP64: 11 FMAs per iteration
+//                instead of 11 Ns (one-range tables; a two-range table re-selects per species and iteration).  The same
+//                warps write the optional outputs of gpuann_chem_step_ex (RR_k, HRR, cp, rho, psi).
+//                "Precision of the scalar math".
 // Barriers the leader's issuers wait on live in the leader and collect arrivals (cluster-scope release) or TMA bytes
 // from BOTH CTAs; barriers that release something to a CTA's own warps are signalled in both CTAs by one multicast
 // tcgen05.commit.

@@ -315,10 +315,8 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
                 if (fa.idx) g = ok4[q] ? (int64_t)fa.idx[g] : 0;
                 g4[q] = ok4[q] ? g : 0;
             }
-#pragma unroll 1
-            for (int u = 0; u < n_units; ++u) {
-                float x[4][8];
-                // loads first (one LDG.128 per feature on the aligned path), arithmetic after
+            // raw loads of one unit (8 features x 4 rows; one LDG.128 per feature on the aligned path)
+            auto load_unit = [&](int u, float (&x)[4][8]) {
 #pragma unroll
                 for (int f = 0; f < 8; ++f) {
                     const int j = u * 8 + f;
@@ -334,6 +332,20 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
                         for (int q = 0; q < 4; ++q) x[q][f] = (j < D && ok4[q]) ? src[g4[q]] : 0.f;
                     }
                 }
+            };
+            // software pipeline over the units: the loads of unit u + 1 are in flight while unit u is transformed (with one
+            // unit at a time the builder needed ~14 k clk per tile -- four exposed memory latencies -- which is longer than
+            // a whole tile of a small net like configs[1])
+            float xa[4][8];
+            load_unit(0, xa);
+#pragma unroll 1
+            for (int u = 0; u < n_units; ++u) {
+                float x[4][8];
+#pragma unroll
+                for (int q = 0; q < 4; ++q)
+#pragma unroll
+                    for (int f = 0; f < 8; ++f) x[q][f] = xa[q][f];
+                if (u + 1 < n_units) load_unit(u + 1, xa);
 #pragma unroll
                 for (int f = 0; f < 8; ++f) {
                     const int j = u * 8 + f;

@@ -38,6 +38,7 @@
 // Barriers the leader's issuer waits on live in the leader and collect arrivals (cluster-scope release) or TMA bytes
 // from BOTH CTAs; barriers that release something to a CTA's own warps are signalled in both CTAs by one multicast
 // tcgen05.commit.
+#include <type_traits>
 #include "common.cuh"
 #include "ptx.cuh"
 
@@ -315,19 +316,26 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
                 if (fa.idx) g = ok4[q] ? (int64_t)fa.idx[g] : 0;
                 g4[q] = ok4[q] ? g : 0;
             }
-            // raw loads of one unit (8 features x 4 rows; one LDG.128 per feature on the aligned path)
+            // raw loads of one unit (8 features x 4 rows; one LDG.128 per feature on the aligned path).  The path is chosen
+            // ONCE per unit, not per feature: per-feature branches keep the compiler from overlapping the eight loads
             auto load_unit = [&](int u, float (&x)[4][8]) {
+                if (vec_ok && all4) {
 #pragma unroll
-                for (int f = 0; f < 8; ++f) {
-                    const int j = u * 8 + f;
-                    const float *src = j == 0 ? fa.T : (j == 1 ? fa.p : fa.Y + (int64_t)(j - 2) * fa.n);
-                    if (j < D && vec_ok && all4) {
-                        const float4 v = *reinterpret_cast<const float4 *>(src + fa.c0 + i0);
+                    for (int f = 0; f < 8; ++f) {
+                        const int j = u * 8 + f;
+                        const float *src = j == 0 ? fa.T : (j == 1 ? fa.p : fa.Y + (int64_t)(j - 2) * fa.n);
+                        float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+                        if (j < D) v = *reinterpret_cast<const float4 *>(src + fa.c0 + i0);
                         x[0][f] = v.x;
                         x[1][f] = v.y;
                         x[2][f] = v.z;
                         x[3][f] = v.w;
-                    } else {
+                    }
+                } else {
+#pragma unroll
+                    for (int f = 0; f < 8; ++f) {
+                        const int j = u * 8 + f;
+                        const float *src = j == 0 ? fa.T : (j == 1 ? fa.p : fa.Y + (int64_t)(j - 2) * fa.n);
 #pragma unroll
                         for (int q = 0; q < 4; ++q) x[q][f] = (j < D && ok4[q]) ? src[g4[q]] : 0.f;
                     }
@@ -346,28 +354,33 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
 #pragma unroll
                     for (int f = 0; f < 8; ++f) x[q][f] = xa[q][f];
                 if (u + 1 < n_units) load_unit(u + 1, xa);
+                // Box-Cox + z-score of the 32 values of the unit.  The lambda = 0 (log) variant is a separate copy of the loop:
+                // a branch per element serialised the eight features (ILP 4 instead of 32: ~3 k clk per unit)
+                auto transform = [&](auto lz) {
+                    constexpr bool kLambdaZero = decltype(lz)::value;
 #pragma unroll
-                for (int f = 0; f < 8; ++f) {
-                    const int j = u * 8 + f;
-                    const float mu = j < D ? fa.pre.mean[j] : 0.f, is = j < D ? fa.pre.inv_std[j] : 0.f;
+                    for (int f = 0; f < 8; ++f) {
+                        const int j = u * 8 + f;
+                        const float mu = j < D ? fa.pre.mean[j] : 0.f, is = j < D ? fa.pre.inv_std[j] : 0.f;
+                        const bool species = j >= 2 && j < D, one = j >= D && j < D + 2;
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        float t = x[q][f];
-                        if (j >= 2 && j < D) {
+                        for (int q = 0; q < 4; ++q) {
+                            float t = x[q][f];
                             // z is rounded to BF16 (2^-9): the approximate lg2 / ex2 pair (2^-22) is ample here;
-                            // Y = 0 still maps to exactly -1/lambda (R1, R2)
+                            // Y = 0 still maps to exactly -1/lambda (R1, R2): lg2(0) = -inf, ex2(-inf) = 0
                             const float Yc = fmaxf(t, 0.f);
-                            if (fa.pre.lambda_zero) t = logf(Yc);
-                            else {
-                                const float uu = Yc > 0.f ? ptx::ex2_approx(fa.pre.lambda * ptx::lg2_approx(Yc)) : 0.f;
-                                t = (uu - 1.f) * fa.pre.inv_lambda;
-                            }
+                            float y;
+                            if (kLambdaZero) y = logf(Yc);
+                            else y = (ptx::ex2_approx(fa.pre.lambda * ptx::lg2_approx(Yc)) - 1.f) * fa.pre.inv_lambda;
+                            t = species ? y : t;
+                            t = (t - mu) * is;
+                            t = one ? 1.f : t;  // multiplies the hi / lo halves of b1 in W1 columns D, D+1
+                            x[q][f] = ok4[q] ? t : 0.f;
                         }
-                        t = (t - mu) * is;
-                        if (j >= D && j < D + 2) t = 1.f;  // multiplies the hi / lo halves of b1 in W1 columns D, D+1
-                        x[q][f] = ok4[q] ? t : 0.f;
                     }
-                }
+                };
+                if (fa.pre.lambda_zero) transform(std::true_type{});
+                else transform(std::false_type{});
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
                     const int rr = 4 * lane + q;

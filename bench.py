@@ -443,7 +443,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
             "cpu_baseline": cpu_baseline,
             "checks": {"finite": ok_finite, "max_abs_sumY_minus_1": sum_dev, "newton_not_converged": int(n_notconv),
                        "degenerate": int(n_degen), "ms_min": min(ms_steps), "ms_median": float(np.median(ms_steps)),
-                       "ms_max": max(ms_steps)},
+                       "ms_max": max(ms_steps), "ms_steps": [round(x, 4) for x in ms_steps]},
         }
         print(json.dumps(line), flush=True)
     if world > 1:

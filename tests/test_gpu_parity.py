@@ -576,3 +576,31 @@ def test_full_size_fp16_and_ex_outputs_sampled():
             assert np.isfinite(v).all(), k
     finally:
         B.gpuann_destroy(ctx)
+
+
+# ------------------------------------------------------------------ shapes other than the five configs
+@pytest.mark.parametrize("ns,hidden", [
+    (10, (144, 336, 48)),      # H1 not a multiple of 64 (zero padded), pass of 336 columns split 176 + 160, narrow layer 3
+    (32, (128, 1008, 416)),    # three passes of 336, the widest layer 3 the tail kernel takes (416), Ns padded to 32
+    (48, (256, 400, 112)),     # the most species the tail kernel takes, D + 2 = 52 features -> four layer-1 K steps
+    (5, (640, 208, 16)),       # one pass of 208 columns, a 16-wide last hidden layer, one 8-species chunk
+    (21, (192, 800, 400, 64)), # FIVE weight matrices: fused kernel, one GEMM layer, tail kernel (row-major h2 path)
+    (60, (256, 256, 128)),     # Ns > 48: no tail kernel -> fused kernel + layer GEMMs + stand-alone update
+    (9, (64, 64)),             # H1 < 128: no fused kernel -> z kernel + layer GEMM + tail kernel (configs[0]'s net in BF16)
+    (50, (96, 80)),            # neither: z kernel + three layer GEMMs + stand-alone update
+])
+def test_other_net_shapes(ns, hidden):
+    """The ABI takes any net: whatever combination of fused kernel / layer GEMM / tail kernel / stand-alone update the
+    shapes select must meet the same BF16-path gates (several tiles + a ragged tail, two chunks)."""
+    cfg = I.Config(f"x{ns}", 9, 4096, ns, tuple(hidden), precision=1)
+    pr = G.prepare(cfg, n=128 * 5 + 61, seed=ns)
+    ctx = G.make_ctx(pr, chunk_cells=512)
+    try:
+        _, variant = B.gpuann_describe(ctx)
+        g = G.run_gpu(ctx, pr)
+        ref = G.run_oracle(pr)
+        w = G.check_all_bf16(g, ref)
+        assert g.stats == (128 * 5 + 61, int((ref.flags & 1).sum()), 0)
+        print(f"Ns={ns} {hidden} [{variant}]: {w}")
+    finally:
+        B.gpuann_destroy(ctx)

@@ -667,6 +667,24 @@ def test_ensemble_output_k_is_net_k_alone_and_matches_numpy():
     assert np.array_equal(r2.o_raw[others], r.o_raw[others]) and not np.array_equal(r2.o_raw[3], r.o_raw[3])
 
 
+def test_newton_stops_when_cp_is_exactly_zero_and_empty_batches_are_fine():
+    """Two boundaries a systematic mutation run of oracle.c found unpinned: c == 0 exactly must stop the iteration (R10:
+    "c <= 0", not "c < 0" -- a division by zero otherwise), and n = 0 is a valid, empty step."""
+    th = _thermo(Ns=3)
+    lo = np.zeros_like(th.nasa_lo)
+    lo[:, 5] = 1.0e3                      # h_k = const, cp_k = 0 for every species
+    Y = np.array([0.2, 0.3, 0.5])
+    T, it, conv = oracle.newton_T(Y, 123.0, 900.0, lo, None, None, th.W)
+    assert T == 900.0 and it == 0 and not conv and np.isfinite(T)
+    pr, h, m = _small_problem(n=8)
+    st = pr.state
+    orc = oracle.Oracle(m)
+    r = orc.chem_step(st.T[:0], st.p[:0], st.Y[:, :0], h[:0], 1e-6)
+    assert r.T_new.shape == (0,) and r.Y_new.shape == (st.Y.shape[0], 0)
+    d = orc.derived(st.T[:0], st.p[:0], st.Y[:, :0], 1e-6, r)
+    assert d.hrr.shape == (0,) and d.rr.shape == (st.Y.shape[0], 0)
+
+
 def test_paper_speedup_arithmetic():
     """context numbers in BASELINE.md are self-consistent (ratio = 32/(1 - reduction))."""
     for red, ratio in read_golden("speedup_arithmetic.txt"):

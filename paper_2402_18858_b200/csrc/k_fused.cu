@@ -525,6 +525,7 @@ k_fused_l1l2(const __grid_constant__ CUtensorMap tmapW1, const __grid_constant__
         while (pass_idx < total_passes) drain();
     }
 
+    ptx::griddep_launch_dependents();  // the tail kernel's CTAs may be scheduled as SMs free up (it waits for this grid's end)
     ptx::tc_fence_before_sync();
     __syncthreads();
     ptx::cluster_sync_all();  // no CTA leaves while its peer may still signal its barriers or the pair's MMAs run

@@ -162,6 +162,8 @@ k_tail(const __grid_constant__ CUtensorMap tmapA /* row-major [rows][K3p] or blo
     __syncthreads();
     ptx::cluster_sync_all();
     ptx::tc_fence_after_sync();
+    // everything above (barriers, TMEM, tensor maps, bias) is independent of the kernel in front; h2 and the state are not
+    ptx::griddep_wait();
     const uint32_t tmem_base = *tmem_slot;
     const uint64_t desc0 = ptx::umma_desc_sw128_kmajor(sbase);
     const uint64_t descA0 = ptx::umma_desc_nosw_kmajor(sbase, 2048, 128);  // blocked A stage: [8 kp][128 rows][16 B]
@@ -644,13 +646,17 @@ cudaError_t launch_tail(Ctx *c, int64_t n, int64_t c0, int64_t cn, float *T, con
     cfg.blockDim = dim3(kTailThreads);
     cfg.dynamicSmemBytes = kTailSmem;
     cfg.stream = s;
-    cudaLaunchAttribute attr[1];
+    cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = 2;
     attr[0].val.clusterDim.y = 1;
     attr[0].val.clusterDim.z = 1;
+    // programmatic dependent launch: a tail CTA may start its prologue on an SM as soon as that SM's CTA of the kernel in
+    // front has exited; the kernel itself waits (griddepcontrol.wait) before it touches h2 or the state
+    attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[1].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = 1;
+    cfg.numAttrs = 2;
     (void)l4;
     // species beyond Ns of the padded range must carry all-zero constants (the kernel's arithmetic is unguarded)
     for (int k = ta.Ns; k < kTailMaxNs; ++k) ta.sA[k] = ta.sC[k] = 0.f;

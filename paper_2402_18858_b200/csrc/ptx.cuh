@@ -214,6 +214,17 @@ __device__ __forceinline__ void umma_commit_multicast(uint64_t *bar, uint16_t ct
                  : "memory");
 }
 
+// ---------------------------------------------------------------- programmatic dependent launch (the tail kernel behind the fused one)
+// griddep_wait: blocks until the grid this one was launched behind (cudaLaunchAttributeProgrammaticStreamSerialization) has
+// completed and its memory is visible; a no-op for a normally launched grid.  griddep_launch_dependents: lets the dependent
+// grid's CTAs start (their prologue) as soon as every CTA of this grid has executed it or exited.
+__device__ __forceinline__ void griddep_wait() {
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+__device__ __forceinline__ void griddep_launch_dependents() {
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
+
 // ---------------------------------------------------------------- tcgen05: TMEM allocation
 // One full warp executes these (.sync.aligned).  ncols: power of two in [32, 512].
 __device__ __forceinline__ void tmem_alloc(uint32_t *smem_result, uint32_t ncols) {

@@ -115,8 +115,8 @@ int gpuann_load_net(gpuann_ctx *ctx, int n_species, int n_layers, const int *siz
  *   sizes    HOST int[L+1]: sizes[0] = 2 + Ns, hidden widths, sizes[L] = 1
  *   weights  HOST, Ns*L pointers: layer l of net k at weights[k*L + l], row-major [sizes[l+1]][sizes[l]]; biases likewise
  * Tensor path only (BF16 or FP16 context) and only shapes the fused + tail kernels run (L = 4, first hidden layer >= 128,
- * last hidden layer <= 416): UNSUPPORTED otherwise.  One step is Ns x (fused kernel + tail kernel) + one update kernel;
- * gpuann_chem_step_ex's optional outputs are not available with an ensemble.  Replaces a net loaded earlier. */
+ * last hidden layer <= 416): UNSUPPORTED otherwise.  One step is Ns x (fused kernel + tail kernel) + one update kernel.
+ * Replaces a net loaded earlier. */
 int gpuann_load_net_ensemble(gpuann_ctx *ctx, int n_species, int n_layers, const int *sizes,
                              const float *const *weights, const float *const *biases,
                              const float *in_mean, const float *in_std,
@@ -170,8 +170,9 @@ typedef struct {
 } gpuann_step_outputs;
 
 /* gpuann_chem_step plus the optional outputs above, computed in the same kernels (no extra pass over the state).
- * out == NULL or all members NULL is exactly gpuann_chem_step.  Errors as gpuann_chem_step, and UNSUPPORTED when an output
- * is requested on a BF16 net that does not run the tail kernel (Ns > 48 or a last hidden layer wider than 416). */
+ * out == NULL or all members NULL is exactly gpuann_chem_step.  Every path provides them: the tail kernel, the FP32 kernel,
+ * and the stand-alone update kernel of nets without a tail kernel and of the per-species ensemble.  Errors as
+ * gpuann_chem_step. */
 int gpuann_chem_step_ex(gpuann_ctx *ctx, int64_t n_cells, float *T, const float *p, float *Y, const float *h,
                         double dt, const gpuann_step_outputs *out, void *stream);
 

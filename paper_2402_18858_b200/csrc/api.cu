@@ -614,7 +614,7 @@ int run_chunk_bf16(Ctx *c, int64_t n, int64_t c0, int64_t cn, const float *T, co
             CU_TRY(c, launch_tail(c, n, c0, cn, nullptr, p, nullptr, nullptr, 1.0, o + (int64_t)k * stride, stride, use_idx, ExtraOut{}, s),
                    "tail kernel");
         }
-        if (!raw_e) CU_TRY(c, launch_post(c, n, c0, cn, out.T, out.Y, out.h, c->o_buf, c->chunk, out.dt, use_idx, s), "update kernel");
+        if (!raw_e) CU_TRY(c, launch_post(c, n, c0, cn, out.T, out.Y, out.h, c->o_buf, c->chunk, out.dt, use_idx, p, out.ex, s), "update kernel");
         return GPUANN_OK;
     }
     int l0 = 0;
@@ -637,7 +637,7 @@ int run_chunk_bf16(Ctx *c, int64_t n, int64_t c0, int64_t cn, const float *T, co
                                  last ? (raw ? out.o_raw : c->o_buf) : nullptr, raw ? out.o_stride : c->chunk, c0, use_idx, s),
                "layer kernel");
     }
-    if (!raw) CU_TRY(c, launch_post(c, n, c0, cn, out.T, out.Y, out.h, c->o_buf, c->chunk, out.dt, use_idx, s), "update kernel");
+    if (!raw) CU_TRY(c, launch_post(c, n, c0, cn, out.T, out.Y, out.h, c->o_buf, c->chunk, out.dt, use_idx, p, out.ex, s), "update kernel");
     return GPUANN_OK;
 }
 
@@ -675,8 +675,6 @@ int gpuann_chem_step_ex(gpuann_ctx *c, int64_t n, float *T, const float *p, floa
         ex.rho = xo->rho;
         ex.psi = xo->psi;
     }
-    if (ex.any() && c->prm.precision != GPUANN_PRECISION_FP32 && (!c->net0.tail.on || !c->ens.empty()))
-        return fail(c, GPUANN_ERR_UNSUPPORTED, "gpuann_chem_step_ex: the extra outputs need the tail kernel (Ns <= 48, last hidden layer <= 416)");
     DeviceGuard g(c->device);
     cudaStream_t s = reinterpret_cast<cudaStream_t>(stream);
     c->last_stream = s;

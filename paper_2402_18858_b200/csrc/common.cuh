@@ -263,7 +263,7 @@ cudaError_t launch_compact(Ctx *c, int64_t n, const float *T, float T_active, cu
 cudaError_t launch_pre_bf16(Ctx *c, int64_t n, int64_t c0, int64_t cn, const float *T, const float *p, const float *Y,
                             bool use_idx, __nv_bfloat16 *z, int Kp, cudaStream_t s);
 cudaError_t launch_post(Ctx *c, int64_t n, int64_t c0, int64_t cn, float *T, float *Y, const float *h, const float *o,
-                        int64_t o_stride, double dt, bool use_idx, cudaStream_t s);
+                        int64_t o_stride, double dt, bool use_idx, const float *p, const ExtraOut &ex, cudaStream_t s);
 cudaError_t launch_enthalpy(Ctx *c, int64_t n, const float *T, const float *Y, float *h_out, cudaStream_t s);
 cudaError_t launch_moments(Ctx *c, int64_t n, int Ns, const float *T, const float *p, const float *Y, double lambda,
                            double *mean_out, double *std_out, cudaStream_t s);

@@ -180,7 +180,8 @@ __global__ void __launch_bounds__(128) k_post_q(int64_t n, int64_t c0, int64_t c
                                                 const float *__restrict__ o, int64_t o_stride, double dt,
                                                 const int32_t *__restrict__ idx, const int32_t *__restrict__ n_active,
                                                 const ThermoDev *__restrict__ thermo_g, Counters *__restrict__ counters,
-                                                float lambda_f, const PostParams pp) {
+                                                float lambda_f, const PostParams pp, const float *__restrict__ p,
+                                                const ExtraOut ex) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     ThermoDev *th = reinterpret_cast<ThermoDev *>(smem_raw);
     {
@@ -268,6 +269,47 @@ __global__ void __launch_bounds__(128) k_post_q(int64_t n, int64_t c0, int64_t c
         }
         if (__all_sync(0xffffffffu, done)) break;
     }
+    if (ex.any()) {
+        // gpuann_chem_step_ex (include/gpuann.h; R19-R21), FP64, species split over the quad like everything above; the
+        // shuffles are warp-wide, so every lane runs along (ex.any() is uniform)
+        double inv_w_in = 0.0, inv_w = 0.0, cpm = 0.0;
+#pragma unroll
+        for (int j = 0; j < NSL; ++j) {
+            const int k = s + 4 * j;
+            if (k < Ns) {
+                inv_w_in = fma((double)fmaxf(yin[j], 0.f), th->inv_W[k], inv_w_in);
+                inv_w = fma(Ys[j], th->inv_W[k], inv_w);
+            }
+        }
+        inv_w_in = quad_sum(inv_w_in);
+        inv_w = quad_sum(inv_w);
+        const double pin = valid ? (double)p[g] : 101325.0;
+        const double rate = valid ? pin / (kRu * T0 * inv_w_in) / dt : 0.0;  // rho of the input state / dt
+        double q = 0.0;
+#pragma unroll
+        for (int j = 0; j < NSL; ++j) {
+            const int k = s + 4 * j;
+            if (k < Ns) {
+                const int r = (two && !(Tn < th->T_mid[k])) ? 1 : 0;
+                const double *cp = th->cp[k][r];
+                const double *hh = th->hh[k][r];
+                const double hk = hh[0] + Tn * (hh[1] + Tn * (hh[2] + Tn * (hh[3] + Tn * (hh[4] + Tn * hh[5]))));
+                const double rr = rate * (Ys[j] - (double)yin[j]);
+                q = fma(-hk, rr, q);
+                cpm = fma(Ys[j], cp[0] + Tn * (cp[1] + Tn * (cp[2] + Tn * (cp[3] + Tn * cp[4]))), cpm);
+                if (valid && ex.rr) ex.rr[(int64_t)k * n + g] = (float)rr;
+            }
+        }
+        q = quad_sum(q);
+        cpm = quad_sum(cpm);
+        if (valid && s == 0) {
+            const double psi = 1.0 / (kRu * inv_w * Tn);
+            if (ex.hrr) ex.hrr[g] = (float)q;
+            if (ex.cp) ex.cp[g] = (float)cpm;
+            if (ex.rho) ex.rho[g] = (float)(pin * psi);
+            if (ex.psi) ex.psi[g] = (float)psi;
+        }
+    }
     if (valid) {
         if (!conv && s == 0) nconv = 1u;
 #pragma unroll
@@ -288,21 +330,21 @@ __global__ void __launch_bounds__(128) k_post_q(int64_t n, int64_t c0, int64_t c
 
 template <int NSL>
 static void launch_post_q(Ctx *c, int64_t n, int64_t c0, int64_t cn, float *T, float *Y, const float *h, const float *o,
-                          int64_t o_stride, double dt, const int32_t *ix, cudaStream_t s) {
+                          int64_t o_stride, double dt, const int32_t *ix, const float *p, const ExtraOut &ex, cudaStream_t s) {
     const unsigned blocks = (unsigned)((cn * 4 + 127) / 128);
     k_post_q<NSL><<<blocks, 128, sizeof(ThermoDev), s>>>(n, c0, cn, T, Y, h, o, o_stride, dt, ix, c->n_active_dev,
-                                                         c->thermo_dev, c->counters, (float)c->lambda, c->post);
+                                                         c->thermo_dev, c->counters, (float)c->lambda, c->post, p, ex);
 }
 
 cudaError_t launch_post(Ctx *c, int64_t n, int64_t c0, int64_t cn, float *T, float *Y, const float *h, const float *o,
-                        int64_t o_stride, double dt, bool use_idx, cudaStream_t s) {
+                        int64_t o_stride, double dt, bool use_idx, const float *p, const ExtraOut &ex, cudaStream_t s) {
     if (cn <= 0) return cudaSuccess;
     LaunchScope ls(c, kClsPost, s);
     const int32_t *ix = use_idx ? c->idx : nullptr;
-    if (c->Ns <= 12) launch_post_q<3>(c, n, c0, cn, T, Y, h, o, o_stride, dt, ix, s);
-    else if (c->Ns <= 24) launch_post_q<6>(c, n, c0, cn, T, Y, h, o, o_stride, dt, ix, s);
-    else if (c->Ns <= 40) launch_post_q<10>(c, n, c0, cn, T, Y, h, o, o_stride, dt, ix, s);
-    else launch_post_q<16>(c, n, c0, cn, T, Y, h, o, o_stride, dt, ix, s);
+    if (c->Ns <= 12) launch_post_q<3>(c, n, c0, cn, T, Y, h, o, o_stride, dt, ix, p, ex, s);
+    else if (c->Ns <= 24) launch_post_q<6>(c, n, c0, cn, T, Y, h, o, o_stride, dt, ix, p, ex, s);
+    else if (c->Ns <= 40) launch_post_q<10>(c, n, c0, cn, T, Y, h, o, o_stride, dt, ix, p, ex, s);
+    else launch_post_q<16>(c, n, c0, cn, T, Y, h, o, o_stride, dt, ix, p, ex, s);
     return cudaGetLastError();
 }
 

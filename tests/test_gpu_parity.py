@@ -525,9 +525,9 @@ def test_small_chunks_ex_fp16_and_ensemble():
             th = pr.prob.thermo
             B.gpuann_load_thermo(ctx, cfg.n_species, th.nasa_lo, th.nasa_hi, th.T_mid, th.W)
             res.append(G.run_gpu(ctx, pr))
-            with pytest.raises(B.GpuannError) as e:      # the optional outputs are not available with an ensemble
-                G.run_gpu_ex(ctx, pr, which=("hrr",))
-            assert e.value.status == 3
+            if chunk:                                    # the optional outputs of an ensemble come from the update kernel
+                g_ex, ex = G.run_gpu_ex(ctx, pr)
+                assert np.array_equal(g_ex.T_new, res[-1].T_new) and np.array_equal(g_ex.Y_new, res[-1].Y_new)
         finally:
             B.gpuann_destroy(ctx)
     assert np.array_equal(res[0].T_new, res[1].T_new) and np.array_equal(res[0].Y_new, res[1].Y_new)
@@ -536,6 +536,24 @@ def test_small_chunks_ex_fp16_and_ensemble():
     st = pr.prob.state
     ref = oracle.Oracle(me).chem_step(st.T, st.p, st.Y, pr.h, cfg.dt)
     G.check_all_bf16(res[0], ref)
+    pe = dataclasses.replace(pr, model=me)
+    print(f"ensemble ex: {G.check_ex(pe, ref, ex, bf16=True)}")
+
+
+@pytest.mark.parametrize("ns,hidden", [(60, (256, 256, 128)), (50, (96, 80))])
+def test_ex_outputs_from_the_standalone_update_kernel(ns, hidden):
+    """Nets without a tail kernel (Ns > 48): RR, HRR, cp, rho, psi come from k_post_q (FP64, species split over a quad)."""
+    cfg = I.Config(f"x{ns}", 9, 4096, ns, tuple(hidden), precision=1)
+    pr = G.prepare(cfg, n=128 * 4 + 33, seed=ns + 1)
+    ctx = G.make_ctx(pr, chunk_cells=256)
+    try:
+        g, ex = G.run_gpu_ex(ctx, pr)
+        ref = G.run_oracle(pr)
+        G.check_T_bf16(g, ref)
+        G.check_Y_bf16(g, ref)
+        print(f"Ns={ns} ex: {G.check_ex(pr, ref, ex, bf16=True)}")
+    finally:
+        B.gpuann_destroy(ctx)
 
 
 def test_full_size_fp16_and_ex_outputs_sampled():

@@ -225,7 +225,9 @@ const char *gpuann_timing_class_name(int cls);
 
 /* Static description of the work one chem_step does, for roofline arithmetic: MACs the tensor path
  * issues per cell including K/N padding (0 on the FP32 path), and the name of the kernel variant chosen
- * for the loaded net ("fp32", "bf16-layerwise", "bf16-fused").  Any out pointer may be NULL. */
+ * for the loaded net: "fp32"; "bf16-fused+tail" (the two-kernel tensor path), "bf16-fused", "bf16-layerwise+tail",
+ * "bf16-layerwise" (fallbacks for shapes one or both kernels do not take); "fp16-fused+tail"; "bf16-ensemble" /
+ * "fp16-ensemble".  Any out pointer may be NULL. */
 int gpuann_describe(const gpuann_ctx *ctx, int64_t *issued_mac_per_cell, const char **variant);
 
 /* Message of the last failure on this context ("" if none).  ctx == NULL returns the message of the last

@@ -126,7 +126,8 @@ __global__ void __launch_bounds__(kFp32Threads) k_chem_fp32(int64_t n, float *__
         }
         if (renormalise<kMaxSpecies>(Ys, Yc, Ns)) ndeg = 1;
         bool conv;
-        const double Tn = newton_T<kMaxSpecies>(Ys, Ns, (double)h[cell], (double)Tin, thermo, pp, &conv);
+        const double Tn = thermo->two_ranges ? newton_T<kMaxSpecies>(Ys, Ns, (double)h[cell], (double)Tin, thermo, pp, &conv)
+                                             : newton_T_mixture<kMaxSpecies>(Ys, Ns, (double)h[cell], (double)Tin, thermo, pp, &conv);
         if (!conv) nconv = 1;
         if (ex.any()) {
             // gpuann_chem_step_ex (include/gpuann.h; R19-R21), FP64, before the inputs are overwritten

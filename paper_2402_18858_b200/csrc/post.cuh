@@ -86,6 +86,37 @@ __device__ __forceinline__ double newton_T(const double (&Y)[MAXNS], int Ns, dou
     return T;
 }
 
+// The same solve for a ONE-RANGE table through the mixture polynomials: C_j = sum_k Y_k c_kj once (11 FMAs per species), then
+// 11 FMAs per iteration instead of 11 Ns -- the FP64 pipe of this part is slow.  Differs from newton_T
+// only by the FP64 rounding of the regrouped sums.
+template <int MAXNS>
+__device__ __forceinline__ double newton_T_mixture(const double (&Y)[MAXNS], int Ns, double h, double T0,
+                                                   const ThermoDev *__restrict__ th, const PostParams &pp, bool *converged) {
+    double Ch[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0}, Cc[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+#pragma unroll 1
+    for (int k = 0; k < Ns; ++k) {
+#pragma unroll
+        for (int m = 0; m < 6; ++m) Ch[m] = fma(Y[k], th->hh[k][0][m], Ch[m]);
+#pragma unroll
+        for (int m = 0; m < 5; ++m) Cc[m] = fma(Y[k], th->cp[k][0][m], Cc[m]);
+    }
+    double T = fmin(fmax(T0, pp.T_min), pp.T_max);
+    bool conv = false;
+    for (int it = 0; it < pp.newton_max_iter; ++it) {
+        const double f = Ch[0] + T * (Ch[1] + T * (Ch[2] + T * (Ch[3] + T * (Ch[4] + T * Ch[5])))) - h;
+        const double c = Cc[0] + T * (Cc[1] + T * (Cc[2] + T * (Cc[3] + T * Cc[4])));
+        if (!(c > 0.0)) break;
+        const double dT = -f / c;
+        T = fmin(fmax(T + dT, pp.T_min), pp.T_max);
+        if (fabs(dT) < pp.newton_tol) {
+            conv = true;
+            break;
+        }
+    }
+    *converged = conv;
+    return T;
+}
+
 // S6: divide by the sum (R8); a vanishing sum falls back to max(Y,0)/sum (counted as degenerate).
 // Ys[] in: Y*; out: Y_new.  Yc[] = clamped inputs.  Returns true if degenerate.
 template <int MAXNS>
@@ -94,8 +125,9 @@ __device__ __forceinline__ bool renormalise(double (&Ys)[MAXNS], const double (&
 #pragma unroll 1
     for (int k = 0; k < Ns; ++k) S += Ys[k];
     if (S > 0.0) {
+        const double rS = 1.0 / S;  // one division per cell; Y* rS differs from Y*/S by <= 1 ulp of FP64
 #pragma unroll 1
-        for (int k = 0; k < Ns; ++k) Ys[k] = Ys[k] / S;
+        for (int k = 0; k < Ns; ++k) Ys[k] = Ys[k] * rS;
         return false;
     }
     double Sc = 0.0;

@@ -209,6 +209,37 @@ int gpuann_enthalpy(gpuann_ctx *ctx, int64_t n_cells, const float *T, const floa
 int gpuann_input_moments(gpuann_ctx *ctx, int64_t n_cells, int n_species, const float *T, const float *p,
                          const float *Y, double lambda, double *mean_out, double *std_out, void *stream);
 
+/* gpuann_input_moments without any device allocation.
+ *
+ * gpuann_input_moments takes its scratch (one FP64 partial sum per thread block and feature, plus the means) from
+ * cudaMalloc and returns it with cudaFree on every call.  Some users of this library cannot afford that once their run
+ * is under way:
+ *   - a flow solver that claimed the GPU's memory for its own fields and pools at start-up: a later cudaMalloc, however
+ *     small, may simply fail, or it fragments what the solver laid out;
+ *   - a time-step loop with other work in flight on the device (halo exchange, the pressure solver on their own
+ *     streams): cudaMalloc and cudaFree wait for the whole device, so each call would stall those streams;
+ *   - codes run under a "no allocation after initialisation" rule (memory-budget audits, week-long production runs).
+ * For them this entry point computes the same statistics with its scratch in a `static __device__` array inside the
+ * library: GPUANN_STATIC_SCRATCH_BYTES bytes that every GPU which loads libgpuann.so holds until the process exits,
+ * whether or not this function is ever called.  It calls no cudaMalloc, cudaFree or other allocating routine.
+ *
+ *   Arguments and results as gpuann_input_moments (T, p, Y DEVICE in; mean_out, std_out HOST double[2+Ns] out;
+ *   synchronises `stream`).  On the same GPU both functions use the same grid and add in the same order.
+ *   Limit: n_species <= GPUANN_STATIC_MAX_SPECIES; anything larger returns GPUANN_ERR_UNSUPPORTED with a message that
+ *   names the limit -- it is never served by a hidden allocation.  n_cells is not limited by the scratch.
+ *   First call on a device: looks up the array's device address (once per device, kept for later calls), which can make
+ *   the CUDA runtime load the library's device code on that GPU.  Make that first call during set-up, before any stream
+ *   capture begins.
+ *   Sharing: there is ONE array per GPU for all contexts, streams and threads, and it keeps what the last call wrote.
+ *   A call overwrites every word before reading it, so nothing has to be cleared in between; but two calls that overlap
+ *   on the same GPU (two streams, two host threads, two contexts) race on it and return garbage.  Serialise them.
+ *   The timing hook (gpuann_timing_enable) counts this function's four launches but does not time them.
+ * Errors: INVALID_ARG (NULLs, n_cells <= 0, n_species < 1, lambda < 0), UNSUPPORTED (limit above), CUDA. */
+#define GPUANN_STATIC_MAX_SPECIES 64
+#define GPUANN_STATIC_SCRATCH_BYTES 271392 /* (512 blocks x 66 features + 66 means + 66 deviations) x 8 bytes */
+int gpuann_input_moments_static(gpuann_ctx *ctx, int64_t n_cells, int n_species, const float *T, const float *p,
+                                const float *Y, double lambda, double *mean_out, double *std_out, void *stream);
+
 /* Number of kernel launches this context has enqueued so far (bench.py reports it as gpu_launches). */
 int64_t gpuann_launch_count(const gpuann_ctx *ctx);
 

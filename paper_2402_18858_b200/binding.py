@@ -23,13 +23,15 @@ GPUANN_ERR_CUDA = 5
 GPUANN_PRECISION_FP32 = 0
 GPUANN_PRECISION_BF16 = 1
 GPUANN_PRECISION_FP16 = 2
+GPUANN_STATIC_MAX_SPECIES = 64
+GPUANN_STATIC_SCRATCH_BYTES = 271392
 
 # every symbol include/gpuann.h declares (tests check that the library exports all of them)
 SYMBOLS = [
     "gpuann_default_params", "gpuann_create", "gpuann_load_net", "gpuann_load_net_ensemble", "gpuann_load_thermo", "gpuann_chem_step",
     "gpuann_chem_step_ex",
     "gpuann_chem_step_host", "gpuann_debug_forward", "gpuann_get_stats", "gpuann_reset_stats", "gpuann_enthalpy",
-    "gpuann_input_moments", "gpuann_launch_count", "gpuann_timing_enable", "gpuann_timing_read",
+    "gpuann_input_moments", "gpuann_input_moments_static", "gpuann_launch_count", "gpuann_timing_enable", "gpuann_timing_read",
     "gpuann_timing_num_classes", "gpuann_timing_class_name", "gpuann_describe", "gpuann_last_error", "gpuann_destroy",
 ]
 
@@ -89,6 +91,8 @@ def lib() -> C.CDLL:
     L.gpuann_enthalpy.argtypes = [vp, i64, vp, vp, vp, vp]
     L.gpuann_input_moments.restype = C.c_int
     L.gpuann_input_moments.argtypes = [vp, i64, C.c_int, vp, vp, vp, dbl, vp, vp, vp]
+    L.gpuann_input_moments_static.restype = C.c_int
+    L.gpuann_input_moments_static.argtypes = [vp, i64, C.c_int, vp, vp, vp, dbl, vp, vp, vp]
     L.gpuann_launch_count.restype = i64
     L.gpuann_launch_count.argtypes = [vp]
     L.gpuann_timing_enable.restype = C.c_int
@@ -241,6 +245,17 @@ def gpuann_input_moments(ctx: int, n_cells: int, n_species: int, T: int, p: int,
     std = np.empty(n_species + 2, dtype=np.float64)
     st = lib().gpuann_input_moments(ctx, int(n_cells), int(n_species), T, p, Y, float(lam), _ptr(mean), _ptr(std),
                                     stream or None)
+    _check(st, ctx)
+    return mean, std
+
+
+def gpuann_input_moments_static(ctx: int, n_cells: int, n_species: int, T: int, p: int, Y: int, lam: float, stream: int = 0):
+    """gpuann_input_moments for callers that must not allocate device memory (scratch in a static device array of the
+    library; at most GPUANN_STATIC_MAX_SPECIES species).  Returns (mean, std) as float64 arrays of 2 + Ns entries."""
+    mean = np.empty(n_species + 2, dtype=np.float64)
+    std = np.empty(n_species + 2, dtype=np.float64)
+    st = lib().gpuann_input_moments_static(ctx, int(n_cells), int(n_species), T, p, Y, float(lam), _ptr(mean), _ptr(std),
+                                           stream or None)
     _check(st, ctx)
     return mean, std
 

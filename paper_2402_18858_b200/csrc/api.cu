@@ -880,6 +880,26 @@ int gpuann_input_moments(gpuann_ctx *c, int64_t n, int n_species, const float *T
     return GPUANN_OK;
 }
 
+// gpuann_input_moments for callers that cannot allocate device memory (include/gpuann.h): scratch in a static __device__
+// array of k_aux.cu, no cudaMalloc / cudaFree, sizes beyond the array are refused
+int gpuann_input_moments_static(gpuann_ctx *c, int64_t n, int n_species, const float *T, const float *p, const float *Y,
+                                double lambda, double *mean_out, double *std_out, void *stream) {
+    if (!c) return fail(nullptr, GPUANN_ERR_INVALID_ARG, "gpuann_input_moments_static: ctx is NULL");
+    if (n <= 0 || n_species < 1 || !T || !p || !Y || !mean_out || !std_out || !(lambda >= 0.0))
+        return fail(c, GPUANN_ERR_INVALID_ARG, "gpuann_input_moments_static: bad argument");
+    if (n_species > GPUANN_STATIC_MAX_SPECIES)
+        return fail(c, GPUANN_ERR_UNSUPPORTED,
+                    "gpuann_input_moments_static: n_species = " + std::to_string(n_species) + " does not fit the static scratch (at most " +
+                        std::to_string(GPUANN_STATIC_MAX_SPECIES) + " species, " + std::to_string(GPUANN_STATIC_SCRATCH_BYTES) +
+                        " bytes); this entry point never allocates");
+    DeviceGuard g(c->device);
+    if (!g.ok) return fail(c, GPUANN_ERR_CUDA, "gpuann_input_moments_static: cudaSetDevice failed");
+    cudaStream_t s = reinterpret_cast<cudaStream_t>(stream);
+    c->last_stream = s;
+    CU_TRY(c, launch_moments_static(c, n, n_species, T, p, Y, lambda, mean_out, std_out, s), "moments kernels (static scratch)");
+    return GPUANN_OK;
+}
+
 int64_t gpuann_launch_count(const gpuann_ctx *c) { return c ? c->launches : 0; }
 
 static void recycle_timed(Ctx *c) {

@@ -267,6 +267,8 @@ cudaError_t launch_post(Ctx *c, int64_t n, int64_t c0, int64_t cn, float *T, flo
 cudaError_t launch_enthalpy(Ctx *c, int64_t n, const float *T, const float *Y, float *h_out, cudaStream_t s);
 cudaError_t launch_moments(Ctx *c, int64_t n, int Ns, const float *T, const float *p, const float *Y, double lambda,
                            double *mean_out, double *std_out, cudaStream_t s);
+cudaError_t launch_moments_static(Ctx *c, int64_t n, int Ns, const float *T, const float *p, const float *Y, double lambda,
+                                  double *mean_out, double *std_out, cudaStream_t s);  // scratch in a static __device__ array
 
 // k_gemm.cu
 cudaError_t gemm_setup(Ctx *c);  // opt-in shared memory etc.

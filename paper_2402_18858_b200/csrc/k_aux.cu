@@ -2,6 +2,8 @@
 // BF16 rows for the tensor path), S4-S7 (update + Newton T-solve) as a stand-alone kernel, and the input-recipe
 // helpers gpuann_enthalpy / gpuann_input_moments.  All state accesses are along the cell index of the SoA
 // fields, i.e. coalesced 128-byte lines per warp.
+#include <mutex>
+
 #include "common.cuh"
 #include "post.cuh"
 
@@ -449,6 +451,89 @@ cudaError_t launch_moments(Ctx *c, int64_t n, int Ns, const float *T, const floa
     cudaFree(partial);
     cudaFree(shift);
     return e;
+}
+
+
+// ================================================================ gpuann_input_moments_static: the same statistics, NO allocation
+// The two-pass moment kernel above needs scratch: one FP64 partial sum per (block, feature) and the D means that pass 2
+// subtracts.  launch_moments gets both from cudaMalloc on every call.  This variant is for callers that cannot do that
+// while they run (include/gpuann.h says who and why), so its scratch is the file-scope array below: part of the
+// library's device image, present on every GPU that loads the library, until the process exits.
+//
+//   layout (doubles): [kStatMaxBlocks * kStatMaxD] partial sums | [kStatMaxD] mean | [kStatMaxD] std
+//   size:             (512 * 66 + 2 * 66) * 8 = 271,392 bytes  (GPUANN_STATIC_SCRATCH_BYTES)
+//
+// Nothing in it has to start at zero: every word a call reads (partial[b][j] for b < blocks, j < D; mean[j]; std[j]) is
+// written earlier in the same call, on the same stream, so whatever the previous call left behind -- more blocks, more
+// species -- is never looked at.  The array is shared by all contexts and all streams of a device: two calls that
+// overlap on the GPU overwrite each other's sums.
+//
+// In HOST code `g_moment_scratch` is only a handle of the symbol, not an address a kernel may dereference: the device
+// address is looked up once per device with cudaGetSymbolAddress (that device current) and passed to the kernels.
+constexpr int kStatMaxBlocks = 512;
+constexpr int kStatMaxD = kMaxSpecies + 2;
+constexpr int kStatMaxDevices = 64;
+constexpr size_t kStatDoubles = (size_t)kStatMaxBlocks * kStatMaxD + 2 * (size_t)kStatMaxD;
+static_assert(kStatDoubles * sizeof(double) == GPUANN_STATIC_SCRATCH_BYTES, "gpuann.h states the size of the static scratch");
+static_assert(kMaxSpecies == GPUANN_STATIC_MAX_SPECIES, "gpuann.h states the species limit of the static scratch");
+
+static __device__ __align__(256) double g_moment_scratch[kStatDoubles];
+
+static std::mutex g_stat_mu;
+static double *g_stat_ptr[kStatMaxDevices] = {};  // device address of g_moment_scratch on device d; nullptr = not looked up
+
+// set-up, once per device; `dev` must be the current device
+static cudaError_t moment_scratch_of_device(int dev, double **out) {
+    if (dev < 0 || dev >= kStatMaxDevices) return cudaErrorInvalidDevice;
+    int cur = -1;
+    cudaError_t e = cudaGetDevice(&cur);
+    if (e != cudaSuccess) return e;
+    if (cur != dev) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lk(g_stat_mu);
+    if (!g_stat_ptr[dev]) {
+        void *ptr = nullptr;
+        e = cudaGetSymbolAddress(&ptr, g_moment_scratch);
+        if (e != cudaSuccess) return e;
+        if (!ptr) return cudaErrorInvalidSymbol;
+        g_stat_ptr[dev] = static_cast<double *>(ptr);
+    }
+    *out = g_stat_ptr[dev];
+    return cudaSuccess;
+}
+
+// Adds the per-block partial sums in block order -- the order, the division and the square root of launch_moments' host
+// loop, all IEEE FP64 -- so both entry points return the same bits for the same grid.  One thread per feature.
+__global__ void __launch_bounds__(128) k_moment_finish(int blocks, int D, int64_t n, int take_sqrt,
+                                                       const double *__restrict__ partial, double *__restrict__ result) {
+    const int j = threadIdx.x;
+    if (j >= D) return;
+    double t = 0.0;
+    for (int b = 0; b < blocks; ++b) t += partial[(size_t)b * D + j];
+    const double q = t / (double)n;
+    result[j] = take_sqrt ? sqrt(q) : q;
+}
+
+cudaError_t launch_moments_static(Ctx *c, int64_t n, int Ns, const float *T, const float *p, const float *Y, double lambda,
+                                  double *mean_out, double *std_out, cudaStream_t s) {
+    const int D = Ns + 2;
+    if (D > kStatMaxD) return cudaErrorInvalidValue;  // the ABI entry has rejected this with a message already
+    int blocks = 2 * (c->sm_count > 0 ? c->sm_count : 148);
+    if (blocks > kStatMaxBlocks) blocks = kStatMaxBlocks;
+    double *scr = nullptr;
+    cudaError_t e = moment_scratch_of_device(c->device, &scr);
+    if (e != cudaSuccess) return e;
+    double *partial = scr, *mean = scr + (size_t)kStatMaxBlocks * kStatMaxD, *sd = mean + kStatMaxD;
+    // (no LaunchScope: with the timing hook on it may create events; these four launches are counted, not timed)
+    c->launches += 4;
+    k_moment_partial<<<blocks, kMomThreads, 0, s>>>(n, D, T, p, Y, lambda, nullptr, 0, partial);
+    k_moment_finish<<<1, 128, 0, s>>>(blocks, D, n, 0, partial, mean);
+    k_moment_partial<<<blocks, kMomThreads, 0, s>>>(n, D, T, p, Y, lambda, mean, 1, partial);
+    k_moment_finish<<<1, 128, 0, s>>>(blocks, D, n, 1, partial, sd);
+    e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaMemcpyAsync(mean_out, mean, sizeof(double) * D, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(std_out, sd, sizeof(double) * D, cudaMemcpyDeviceToHost, s);
+    const cudaError_t e2 = cudaStreamSynchronize(s);
+    return e != cudaSuccess ? e : e2;
 }
 
 }  // namespace gpuann

@@ -65,7 +65,9 @@ typedef enum {
 #define GPUANN_PRECISION_BF16 1 /* tcgen05 BF16 x BF16 -> FP32 MLP, activations rounded to BF16 (configs[1..4]) */
 #define GPUANN_PRECISION_FP16 2 /* the same kernels with FP16 weights and activations, FP32 accumulate: the half precision
                                    the paper infers in.  Weights are rounded to FP16
-                                   (values that are FP16-representable are used exactly; |w| must stay below 65504).
+                                   after the factor 1/2 that hidden-layer weights are stored with: an FP16-representable
+                                   weight is used exactly unless |w| < 2^-13 (w/2 is then subnormal and may lose its last
+                                   bit); |w/2| (first layer: |w|, |b|) must stay below 65520 or the load is INVALID_ARG.
                                    Only nets that run the fused + tail kernels (4 weight matrices, Ns <= 48,
                                    last hidden layer <= 416, first hidden layer >= 128): UNSUPPORTED otherwise */
 
@@ -101,9 +103,12 @@ int gpuann_create(const gpuann_params *params, gpuann_ctx **out);
  *   in_mean, in_std    HOST float[2+Ns]: z-score statistics of {T, p, y_k} (R4); in_std > 0
  *   out_mean, out_std  HOST float[Ns]: de-normalisation of the output, units 1/s (R3)
  *   lambda     Box-Cox exponent (0.1); lambda = 0 selects the log/exp branch of Eq. 7
- * GELU is applied after every layer but the last.  May be called again to replace the net.
+ * GELU is applied after every layer but the last.  May be called again to replace the net: a load that
+ * fails with INVALID_ARG or UNSUPPORTED leaves the net loaded earlier in place and usable; one that fails with ALLOC or
+ * CUDA leaves the context without a net (NOT_READY until a load succeeds).  The same holds for gpuann_load_net_ensemble.
  * Errors: INVALID_ARG (NULLs, sizes[0] != 2+Ns, sizes[L] != Ns, width < 1, in_std <= 0 or not finite,
- * lambda < 0, n_species differs from a loaded thermo table), UNSUPPORTED (limits above), ALLOC, CUDA. */
+ * lambda < 0, n_species differs from a loaded thermo table, a weight or bias that is not finite or -- on the tensor
+ * path -- overflows BF16 / FP16 once stored), UNSUPPORTED (limits above), ALLOC, CUDA. */
 int gpuann_load_net(gpuann_ctx *ctx, int n_species, int n_layers, const int *sizes,
                     const float *const *weights, const float *const *biases,
                     const float *in_mean, const float *in_std,

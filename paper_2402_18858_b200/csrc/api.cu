@@ -223,6 +223,10 @@ int build_subnet(Ctx *c, SubNet &sn, int n_out, int n_layers, const int *sizes, 
     }
     const bool one_buffer = fused && tail && n_layers == 4;
     for (int l = fused ? 2 : 0; l < n_layers; ++l) {
+        // tmapA is read by the layer kernel and by the tail kernel's row-major input.  Not encoded where nothing reads it:
+        // the last layer under a tail kernel (h3 stays in shared memory), and the tail kernel's input when it is the
+        // blocked h2 (tmapAb below) -- in that mode act[1] does not even exist.
+        if (tail && (l == n_layers - 1 || (l == n_layers - 2 && one_buffer))) continue;
         LayerBf16 &ly = sn.lay[l];
         std::string terr;
         if (!encode_tmap_bf16(&ly.tmapA, c->act[l & 1], (uint64_t)ly.Kp, (uint64_t)chunk, (uint64_t)ly.Kp * 2, 128, &terr))
@@ -338,7 +342,66 @@ int gpuann_create(const gpuann_params *params, gpuann_ctx **out) {
     return GPUANN_OK;
 }
 
-// validation + the parameter blocks every path shares (S1-S2 statistics, S4-S7 constants); frees the previous net
+// which kernels would run a net of these sizes, and whether this context's precision takes it (the same decisions as
+// plan_and_alloc / build_subnet / the FP32 branch of gpuann_load_net, taken here without touching the context)
+static int check_net_supported(gpuann_ctx *c, const char *fn, int n_layers, const int *sizes, int n_out, int n_nets, int maxw) {
+    const std::string f(fn);
+    if (c->prm.precision == GPUANN_PRECISION_FP32) {
+        if (n_nets > 1) return fail(c, GPUANN_ERR_UNSUPPORTED, f + ": tensor path only (BF16 or FP16 context)");
+        // fp32_smem_bytes: two activation rows of the widest layer for 8 cells must fit 200 KB of shared memory
+        if (2ull * (size_t)maxw * 8 * sizeof(float) > 200 * 1024)
+            return fail(c, GPUANN_ERR_UNSUPPORTED, f + ": layer too wide for the FP32 path (max width 3200)");
+        return GPUANN_OK;
+    }
+    const bool fused = n_layers >= 3 && fused_supported(sizes[0], sizes[1], pad16(sizes[2]));
+    const bool tail = n_layers >= (fused ? 4 : 2) && tail_supported(pad16(sizes[n_layers - 2]), pad16(sizes[n_layers - 1]), n_out);
+    const bool two_kernels = fused && tail && n_layers == 4;
+    if (c->prm.precision == GPUANN_PRECISION_FP16 && !two_kernels)
+        return fail(c, GPUANN_ERR_UNSUPPORTED, f + ": GPUANN_PRECISION_FP16 needs a net the fused + tail kernels run (4 weight matrices)");
+    if (n_nets > 1 && !two_kernels)
+        return fail(c, GPUANN_ERR_UNSUPPORTED,
+                    f + ": every net must run the fused + tail kernels (4 weight matrices, first hidden layer >= 128, last <= 416)");
+    return GPUANN_OK;
+}
+
+// weights and biases must be finite, and on the tensor path they must stay finite in the operand type: a hidden-layer
+// weight is stored as BF16 / FP16 of w/2 (build_subnet), the first-layer bias of the fused kernel as two such values.
+// An inf operand would make the raw output NaN, every cell would take the vanishing-sum fallback and the chemistry would
+// freeze with nothing but a counter to show for it -- so it is an error here.
+static int check_net_values(gpuann_ctx *c, const char *fn, int n_layers, const int *sizes, int n_out, int n_nets,
+                            const float *const *weights, const float *const *biases) {
+    (void)n_out;
+    const std::string f(fn);
+    const int prec = c->prm.precision;
+    const bool tensor = prec != GPUANN_PRECISION_FP32;
+    const bool f16 = prec == GPUANN_PRECISION_FP16;
+    const bool fused = tensor && n_layers >= 3 && fused_supported(sizes[0], sizes[1], pad16(sizes[2]));
+    auto overflows = [f16](float v) {
+        return f16 ? (f32_to_f16_rne(v) & 0x7C00u) == 0x7C00u : (f32_to_bf16_rne(v) & 0x7F80u) == 0x7F80u;
+    };
+    const char *type = f16 ? "FP16" : "BF16";
+    for (int k = 0; k < n_nets; ++k)
+        for (int l = 0; l < n_layers; ++l) {
+            const float *w = weights[(size_t)k * n_layers + l], *b = biases[(size_t)k * n_layers + l];
+            const size_t cnt = (size_t)sizes[l] * sizes[l + 1];
+            const float wscale = l >= 1 ? 0.5f : 1.f;
+            const std::string where = (n_nets > 1 ? " of net " + std::to_string(k) : std::string()) + " in layer " + std::to_string(l);
+            for (size_t i = 0; i < cnt; ++i) {
+                if (!finite_f(w[i])) return fail(c, GPUANN_ERR_INVALID_ARG, f + ": weight " + std::to_string(i) + where + " is not finite");
+                if (tensor && overflows(wscale * w[i]))
+                    return fail(c, GPUANN_ERR_INVALID_ARG, f + ": weight " + std::to_string(i) + where + " overflows " + type);
+            }
+            for (int j = 0; j < sizes[l + 1]; ++j) {
+                if (!finite_f(b[j])) return fail(c, GPUANN_ERR_INVALID_ARG, f + ": bias " + std::to_string(j) + where + " is not finite");
+                if (fused && l == 0 && overflows(b[j]))
+                    return fail(c, GPUANN_ERR_INVALID_ARG, f + ": bias " + std::to_string(j) + where + " overflows " + type);
+            }
+        }
+    return GPUANN_OK;
+}
+
+// validation + the parameter blocks every path shares (S1-S2 statistics, S4-S7 constants); frees the previous net once
+// nothing can refuse the new one any more
 static int load_prologue(gpuann_ctx *c, const char *fn, int n_species, int n_layers, const int *sizes, int n_out, int n_nets,
                          const float *const *weights, const float *const *biases, const float *in_mean,
                          const float *in_std, const float *out_mean, const float *out_std, double lambda) {
@@ -367,6 +430,16 @@ static int load_prologue(gpuann_ctx *c, const char *fn, int n_species, int n_lay
     if (!(lambda >= 0.0) || !std::isfinite(lambda)) return fail(c, GPUANN_ERR_INVALID_ARG, std::string(fn) + ": lambda must be >= 0");
     if (c->thermo_loaded && c->thermo_Ns != n_species)
         return fail(c, GPUANN_ERR_INVALID_ARG, std::string(fn) + ": n_species differs from the loaded thermo table");
+
+    // Every check that can REFUSE the net runs before the net loaded earlier is freed, so a load that fails with
+    // INVALID_ARG or UNSUPPORTED leaves that net in place and usable (include/gpuann.h).  Only ALLOC / CUDA failures
+    // further down leave the context without a net.
+    {
+        const int rc = check_net_supported(c, fn, n_layers, sizes, n_out, n_nets, maxw);
+        if (rc != GPUANN_OK) return rc;
+        const int rc2 = check_net_values(c, fn, n_layers, sizes, n_out, n_nets, weights, biases);
+        if (rc2 != GPUANN_OK) return rc2;
+    }
 
     DeviceGuard g(c->device);
     cudaDeviceSynchronize();

@@ -429,6 +429,68 @@ def test_fp16_unsupported_shapes_fail_loudly():
         B.gpuann_destroy(ctx)
 
 
+def test_refused_load_keeps_the_previous_net_and_bad_weights_are_refused():
+    """include/gpuann.h, gpuann_load_net: a load that fails with UNSUPPORTED or INVALID_ARG leaves the net loaded earlier
+    in place (the step afterwards is bit-identical); weights / biases that are not finite or overflow the operand type are
+    INVALID_ARG instead of a silently frozen chemistry."""
+    pr = G.prepare(I.get_config("c1h"), n=128 * 3 + 5, seed=3)
+    net, cfg = pr.prob.net, pr.prob.cfg
+    small = G.prepare(I.get_config("c0"), n=64)
+
+    def load(ctx, weights=None, biases=None):
+        B.gpuann_load_net(ctx, cfg.n_species, net.sizes, net.weights if weights is None else weights,
+                          net.biases if biases is None else biases, pr.in_mean, pr.in_std, pr.prob.out_mean, pr.prob.out_std, cfg.lam)
+
+    def edited(arrs, l, idx, value):
+        out = [np.array(a, dtype=np.float32, copy=True) for a in arrs]
+        out[l].reshape(-1)[idx] = value
+        return out
+
+    ctx = G.make_ctx(pr)                     # FP16 context, 23-400-200-100-21 on the fused + tail kernels
+    try:
+        g0 = G.run_gpu(ctx, pr, want_raw=False)
+        # (1) a shape the FP16 path does not take
+        rng = np.random.default_rng(2)
+        sz = [23, 64, 64, 64, 21]             # first hidden layer < 128: not a net of the fused kernel
+        ws = [rng.standard_normal((sz[l + 1], sz[l])).astype(np.float32) * 0.1 for l in range(4)]
+        bs = [np.zeros(sz[l + 1], dtype=np.float32) for l in range(4)]
+        with pytest.raises(B.GpuannError) as e:
+            B.gpuann_load_net(ctx, 21, sz, ws, bs, pr.in_mean, pr.in_std, pr.prob.out_mean, pr.prob.out_std, cfg.lam)
+        assert e.value.status == B.GPUANN_ERR_UNSUPPORTED
+        # (2) NaN weight, inf bias, FP16 overflow of w/2 in a hidden layer and of a first-layer bias
+        for weights, biases, what in (
+                (edited(net.weights, 2, 17, np.nan), None, "not finite"),
+                (None, edited(net.biases, 3, 4, np.inf), "not finite"),
+                (edited(net.weights, 1, 5, 140000.0), None, "overflows FP16"),
+                (None, edited(net.biases, 0, 7, -70000.0), "overflows FP16")):
+            with pytest.raises(B.GpuannError) as e:
+                load(ctx, weights, biases)
+            assert e.value.status == B.GPUANN_ERR_INVALID_ARG and what in e.value.message, e.value.message
+        # 65504 = the largest FP16 value is fine as a first-layer weight, and w = 131008 is as a hidden-layer weight (w/2 = 65504)
+        _, variant = B.gpuann_describe(ctx)
+        assert variant == "fp16-fused+tail"
+        g1 = G.run_gpu(ctx, pr, want_raw=False)
+        assert np.array_equal(g0.T_new, g1.T_new) and np.array_equal(g0.Y_new, g1.Y_new)
+        load(ctx, edited(net.weights, 1, 5, 131008.0))     # accepted: replaces the net
+    finally:
+        B.gpuann_destroy(ctx)
+
+    # FP32 context: the ensemble is refused, the FP32 net stays
+    ctx = G.make_ctx(small)
+    try:
+        g0 = G.run_gpu(ctx, small, want_raw=False)
+        sz = list(small.prob.net.sizes[:-1]) + [1]
+        ws = [[w if l < len(sz) - 2 else w[:1] for l, w in enumerate(small.prob.net.weights)] for _ in range(9)]
+        bs = [[b if l < len(sz) - 2 else b[:1] for l, b in enumerate(small.prob.net.biases)] for _ in range(9)]
+        with pytest.raises(B.GpuannError) as e:
+            B.gpuann_load_net_ensemble(ctx, 9, sz, ws, bs, small.in_mean, small.in_std, small.prob.out_mean, small.prob.out_std, 0.1)
+        assert e.value.status == B.GPUANN_ERR_UNSUPPORTED
+        g1 = G.run_gpu(ctx, small, want_raw=False)
+        assert np.array_equal(g0.T_new, g1.T_new) and np.array_equal(g0.Y_new, g1.Y_new)
+    finally:
+        B.gpuann_destroy(ctx)
+
+
 # ------------------------------------------------------------------ per-species ensemble (SURVEY 8f NEXT-1; PAPER.md:103; R24)
 @pytest.mark.parametrize("name,n", [("c2", 128 * 6 + 19), ("c1", 128 * 20 + 3), ("c4", 128 * 8 + 77)])
 def test_ensemble_of_one_output_nets(name, n):

@@ -201,6 +201,7 @@ struct Ctx {
     std::vector<cudaEvent_t> slice_events;
     cudaStream_t last_stream = nullptr;
     int64_t launches = 0;
+    int last_cls = -1;  // KernelClass of the launch enqueued last (LaunchScope); launch_tail decides on it whether PDL is safe
 
     // per-kernel-class device timing (gpuann_timing_enable / gpuann_timing_read): CUDA events around every launch
     bool timing = false;
@@ -232,6 +233,7 @@ struct LaunchScope {
     cudaEvent_t e1 = nullptr;
     LaunchScope(Ctx *ctx, int cls, cudaStream_t stream, int n_launches = 1) : c(ctx), s(stream) {
         c->launches += n_launches;
+        c->last_cls = cls;
         if (!c->timing) return;
         cudaEvent_t ev[2] = {nullptr, nullptr};
         for (int i = 0; i < 2; ++i) {

@@ -119,6 +119,10 @@ k_tail(const __grid_constant__ CUtensorMap tmapA /* row-major [rows][K3p] or blo
     const uint32_t sbase = ptx::smem_u32(smem);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
+    // *ta.n_active (written by k_compact_scan) and bias3 (written at load time) are read BEFORE griddepcontrol.wait.
+    // That is safe only because launch_tail asks for programmatic dependent launch solely behind a kernel that was itself
+    // launched with full stream ordering (fused / pre / layer kernel): no tail CTA can start before that kernel has
+    // started, i.e. before everything in front of it -- the compaction -- has completed.  launch_tail enforces this.
     int64_t rows = ta.rows;
     if (ta.n_active) {
         int64_t r = (int64_t)*ta.n_active - ta.c0;
@@ -640,6 +644,10 @@ cudaError_t launch_tail(Ctx *c, int64_t n, int64_t c0, int64_t cn, float *T, con
     const int64_t tiles = (cn + kTM - 1) / kTM;
     int grid = (int)(tiles < c->sm_count ? tiles : c->sm_count);
     grid = (grid + 1) & ~1;
+    // INVARIANT of the kernel's prologue (it reads *n_active before griddepcontrol.wait): PDL only directly behind a kernel
+    // of this context that was launched with full stream ordering and writes neither n_active nor the thermo / bias
+    // tables.  Behind anything else (the compaction kernels, another tail kernel, nothing) the launch is an ordinary one.
+    const bool pdl = c->last_cls == kClsFused || c->last_cls == kClsPre || (c->last_cls >= kClsLayer0 && c->last_cls < kClsLayer0 + kMaxLayers);
     LaunchScope ls(c, kClsTail, s);
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)grid);
@@ -656,7 +664,7 @@ cudaError_t launch_tail(Ctx *c, int64_t n, int64_t c0, int64_t cn, float *T, con
     attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[1].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = 2;
+    cfg.numAttrs = pdl ? 2 : 1;
     (void)l4;
     // species beyond Ns of the padded range must carry all-zero constants (the kernel's arithmetic is unguarded)
     for (int k = ta.Ns; k < kTailMaxNs; ++k) ta.sA[k] = ta.sC[k] = 0.f;

@@ -49,21 +49,46 @@ def load_peaks():
     return dict(FALLBACK_PEAKS), "fallback (B200_PROFILING.md)"
 
 
-def dram_bytes_from_profiles(kernel_class: str, config_index: int, n_cells: int):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch from profiles/ncu_dram_bytes.csv (None if no row matches)."""
+def csrc_sha() -> str:
+    """First 16 hex digits of the SHA-256 over the kernel sources (paper_2402_18858_b200/csrc/*.cu, *.cuh and
+    include/gpuann.h, in name order, each as name + NUL + bytes): names the kernels an ncu capture was taken from.  The
+    sources, not the built library, because -lineinfo puts the build directory into the .so."""
+    import hashlib
+    h = hashlib.sha256()
+    csrc = ROOT / "paper_2402_18858_b200" / "csrc"
+    files = sorted(list(csrc.glob("*.cu")) + list(csrc.glob("*.cuh")), key=lambda f: f.name) + [ROOT / "include" / "gpuann.h"]
+    for f in files:
+        h.update(f.name.encode() + b"\0" + f.read_bytes())
+    return h.hexdigest()[:16]
+
+
+def dram_capture_from_profiles(kernel_class: str, config_index: int, n_cells: int, sha: str = None):
+    """The row of profiles/ncu_dram_bytes.csv (ncu --set full: dram__bytes_read.sum, dram__bytes_write.sum per launch) for
+    this kernel class, configuration and cell count, as {"bytes", "source", "csrc_sha", "current"}; None if there is
+    none.  "current" says whether the capture was taken from the kernel sources of this tree (csrc_sha())."""
     p = ROOT / "profiles" / "ncu_dram_bytes.csv"
     if not p.exists():
         return None
+    sha = csrc_sha() if sha is None else sha
     try:
         rows = [l.strip().split(",") for l in p.read_text().splitlines() if l.strip() and not l.startswith("#")]
         hdr = rows[0]
         for r in rows[1:]:
             d = dict(zip(hdr, r))
             if d["kernel_class"] == kernel_class and int(d["config"]) == config_index and int(d["cells"]) == n_cells:
-                return float(d["dram_bytes_read"]) + float(d["dram_bytes_write"])
+                return {"bytes": float(d["dram_bytes_read"]) + float(d["dram_bytes_write"]), "source": d.get("source"),
+                        "csrc_sha": d.get("csrc_sha"), "current": d.get("csrc_sha") == sha}
     except Exception:
         return None
     return None
+
+
+def dram_bytes_from_profiles(kernel_class: str, config_index: int, n_cells: int, sha: str = None):
+    """roofline.traffic: the captured DRAM bytes per launch, or None when there is no capture of exactly this kernel class,
+    configuration and cell count TAKEN FROM THE KERNEL SOURCES OF THIS TREE (a capture of older kernels is not reported as
+    if it were current)."""
+    cap = dram_capture_from_profiles(kernel_class, config_index, n_cells, sha)
+    return cap["bytes"] if cap and cap["current"] else None
 
 
 # ------------------------------------------------------------------ clocks
@@ -332,8 +357,11 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     achieved = flop_step / (dom_ms_per_step * 1e-3) / 1e12
     # DRAM bytes of the dominant kernel per launch: dram__bytes_read.sum + dram__bytes_write.sum of the committed
     # `ncu --set full` capture of exactly this kernel class, configuration and cell count (profiles/ncu_dram_bytes.csv,
-    # written from the .ncu-rep by hand with its command beside it); null when no capture matches
-    traffic = dram_bytes_from_profiles(dom_name, cfg.index, n) if not args.chunk else None
+    # written from the .ncu-rep with its command beside it, each row carrying the csrc_sha() of the sources it was
+    # taken from); null when no capture matches or the capture is of other sources
+    sha_now = csrc_sha()
+    capture = dram_capture_from_profiles(dom_name, cfg.index, n, sha_now) if not args.chunk else None
+    traffic = capture["bytes"] if capture and capture["current"] else None
     # what each kernel class must move by design (bytes per step): state in / out, h2 out / in, weights once
     h2_bytes = 2.0 * (sizes[2] if len(sizes) > 3 else 0) * n_act_per_step
     by_design = {"state_algorithmic": float(cfg.state_bytes_per_cell) * n_act_per_step,
@@ -342,6 +370,11 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     roofline = {
         "bound": "tensor", "kernel": dom_name, "achieved": achieved, "peak": peaks["bf16_tflops"], "unit": "TFLOP/s",
         "frac": achieved / peaks["bf16_tflops"], "traffic": traffic, "traffic_by_design": by_design,
+        # where `traffic` comes from: the committed ncu capture and the kernel sources it was taken from; when those are
+        # not this tree's sources, traffic is null and traffic_stale carries the old figure for context only
+        "traffic_source": capture["source"] if capture else None,
+        "traffic_csrc_sha": capture["csrc_sha"] if capture else None, "csrc_sha": sha_now,
+        "traffic_stale": capture["bytes"] if capture and not capture["current"] else None,
         "peak_source": peak_src + ", burst",
         "launches_per_step": dom_cnt / args.steps, "ms_per_step_in_kernel": dom_ms_per_step,
         "share_of_step": dom_ms_per_step / step_ms_sum if step_ms_sum > 0 else None,

@@ -66,9 +66,16 @@ def test_single_rank_aggregation_is_identity():
 
 def test_roofline_traffic_comes_from_the_tracked_ncu_table():
     """bench.py's roofline.traffic is read from profiles/ncu_dram_bytes.csv (ncu --set full captures), never a literal in
-    the code; a configuration without a capture yields None."""
+    the code; a configuration without a capture yields None, and so does a capture taken from other kernel sources than
+    this tree's (each row names the csrc_sha() it was measured on)."""
     import bench
-    t = bench.dram_bytes_from_profiles("bf16_fused", 2, 1048576)
-    assert t is not None and 1.5e9 < t < 2.0e9          # state in + h2 out of the fused kernel at configs[2]
+    cap = bench.dram_capture_from_profiles("bf16_fused", 2, 1048576)
+    assert cap is not None and 1.5e9 < cap["bytes"] < 2.0e9   # state in + h2 out of the fused kernel at configs[2]
+    assert cap["source"].startswith("profiles/") and len(cap["csrc_sha"]) == 16
+    sha = bench.csrc_sha()
+    assert len(sha) == 16 and int(sha, 16) >= 0
+    # a capture of these sources is reported, one of other sources is not
+    assert bench.dram_bytes_from_profiles("bf16_fused", 2, 1048576, sha=cap["csrc_sha"]) == cap["bytes"]
+    assert bench.dram_bytes_from_profiles("bf16_fused", 2, 1048576, sha="0" * 16) is None
     assert bench.dram_bytes_from_profiles("bf16_fused", 3, 4194304) is None
     assert bench.dram_bytes_from_profiles("bf16_tail", 2, 12345) is None

@@ -4,7 +4,10 @@ oracle, run the CUDA path through the C ABI (ctypes binding) and the oracle on t
 Tolerances (BASELINE.json north_star):
   FP32 path: |Y - Y_ref| <= 1e-5 |Y_ref| + 1e-10, max |T - T_ref| <= 1e-3 K
   BF16 path: per output column ||o - o_ref||_2 <= 2e-2 ||o_ref||_2 and max|o - o_ref| <= 2e-2 max|o_ref|,
-             max |T - T_ref| <= 0.5 K, |Y - Y_ref| <= 2e-3 |Y_ref| + 1e-10 (R18)
+             max |T - T_ref| <= 0.5 K, |Y - Y_ref| <= 2e-3 |Y_ref| + 1e-10 (R18), and -- the gates that bite --
+             on the UPDATE dY = Y_new - Y_in/sum(Y_in), per species over the batch (R18'):
+             ||Y - Y_ref||_2 <= 2e-2 ||dY_ref||_2 and max|Y - Y_ref| <= 2e-2 max|dY_ref| (+ a floor of 2 FP32 ulps);
+             RR_k likewise against RR_ref,k; HRR per cell within rho cp 0.5 K / dt and 3e-2 of ||HRR_ref||_2 (R22')
   both:      max |sum_k Y_new - 1| <= 1e-6 (FP64 sum of the stored FP32 values)
 """
 from __future__ import annotations
@@ -113,8 +116,10 @@ def run_gpu(ctx: int, pr: Prepared, T=None, p=None, Y=None, h=None, want_raw: bo
 def run_oracle(pr: Prepared, T=None, p=None, Y=None, h=None, dt: Optional[float] = None):
     st = pr.prob.state
     o = oracle.Oracle(pr.model)
-    return o.chem_step(st.T if T is None else T, st.p if p is None else p, st.Y if Y is None else Y,
-                       pr.h if h is None else h, pr.prob.cfg.dt if dt is None else dt)
+    ref = o.chem_step(st.T if T is None else T, st.p if p is None else p, st.Y if Y is None else Y,
+                      pr.h if h is None else h, pr.prob.cfg.dt if dt is None else dt)
+    ref.Y_in = st.Y if Y is None else Y     # the update gates (R18') are stated on Y_new - Y_in / sum Y_in
+    return ref
 
 
 def run_oracle_all_active(pr: Prepared):
@@ -187,11 +192,53 @@ def check_Y_bf16(g: GpuResult, ref, mask=None, lam: float = 0.1):
     return worst
 
 
+def update_of(Y_new: np.ndarray, Y_in: np.ndarray) -> np.ndarray:
+    """dY = Y_new - max(Y_in, 0) / sum_k max(Y_in, 0): what the step changes (S1 reads Y < 0 as 0, R2; S6 renormalises)."""
+    Yc = np.maximum(np.asarray(Y_in, dtype=np.float64), 0.0)
+    return np.asarray(Y_new, dtype=np.float64) - Yc / Yc.sum(axis=0, keepdims=True)
+
+
+def norms_against(d: np.ndarray, ref: np.ndarray, floor: np.ndarray, gate: float):
+    """Per row k (a species) over the batch: ||d_k||_2 / (gate ||ref_k||_2 + ||floor_k||_2) and
+    max|d_k| / (gate max|ref_k| + max floor_k); rows whose allowance is 0 must have d = 0.  Returns the two worst ratios."""
+    if d.size == 0:
+        return 0.0, 0.0
+    a2 = gate * np.sqrt((ref * ref).sum(axis=1)) + np.sqrt((floor * floor).sum(axis=1))
+    am = gate * np.abs(ref).max(axis=1) + floor.max(axis=1)
+    e2, em = np.sqrt((d * d).sum(axis=1)), np.abs(d).max(axis=1)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        r2 = np.where(a2 > 0, e2 / a2, np.where(e2 > 0, np.inf, 0.0))
+        rm = np.where(am > 0, em / am, np.where(em > 0, np.inf, 0.0))
+    return float(r2.max()), float(rm.max())
+
+
+def check_Y_update(g: GpuResult, ref, mask=None, gate: float = 2e-2):
+    """The gate on Y_new that bites on the tensor path (R18').  north_star states 2e-2 on the raw output o (R13:
+    per output column, rel-L2 and max against the column's largest entry).  The species update is, to first order, LINEAR
+    in o (dY_k ~ Y_k^(1-lambda) dt sigma_k o_k, then the renormalisation), so the same 2e-2 in the same two norms is what
+    that statement allows on the UPDATE dY_k = Y_new,k - Y_in,k / sum Y_in, per species k over the batch:
+        ||Y_k - Y_ref,k||_2 <= 2e-2 ||dY_ref,k||_2 + ||floor_k||_2,   max|Y_k - Y_ref,k| <= 2e-2 max|dY_ref,k| + max floor_k
+    with floor = 2.4e-7 |Y_ref| + 1e-30 = 2 FP32 ulps: the tensor path renormalises in FP32 (sum, reciprocal, product, store:
+    S6), which is all that is left where the update vanishes (the degenerate-sum fallback returns max(Y,0)/sum: dY = 0);
+    it is ~1 % of the allowance at a typical update of 1e-3 |Y|.  (R18's element-wise 2e-3 |Y| is 1-2 x the update itself
+    on these inputs: it bounds blow-ups, not the update.)  Returns the worse of the two ratios."""
+    Y_in = getattr(ref, "Y_in", None)
+    assert Y_in is not None, "the oracle result carries no Y_in (use gpu_common.run_oracle / subset, or set ref.Y_in)"
+    sel = slice(None) if mask is None else mask
+    act = (ref.flags[sel] & 4) == 0          # skipped cells are compared bit for bit elsewhere
+    Yg, Yr = g.Y_new.astype(np.float64)[:, sel][:, act], ref.Y_new[:, sel][:, act]
+    dref = update_of(Yr, np.asarray(Y_in)[:, sel][:, act])
+    r2, rm = norms_against(Yg - Yr, dref, 2.4e-7 * np.abs(Yr) + 1e-30, gate)
+    assert r2 <= 1.0, f"Y_new update: per-species L2 error / allowance = {r2:.3f} (allowance = {gate:g} ||dY_ref||_2 + store floor)"
+    assert rm <= 1.0, f"Y_new update: per-species max error / allowance = {rm:.3f} (allowance = {gate:g} max|dY_ref| + store floor)"
+    return max(r2, rm)
+
+
 def check_all_bf16(g: GpuResult, ref, mask=None, raw_ref=None, lam: float = 0.1):
     """Every BF16-path gate at once; returns a dict of the worst figures."""
     l2, mx = check_raw_bf16(g.o_raw, (ref if raw_ref is None else raw_ref).o_raw)
     return {"raw_l2": l2, "raw_max": mx, "dT": check_T_bf16(g, ref, mask), "Y": check_Y_bf16(g, ref, mask, lam),
-            "sumY": check_sumY(g.Y_new, mask)}
+            "dY": check_Y_update(g, ref, mask), "sumY": check_sumY(g.Y_new, mask)}
 
 
 def sample_indices(n, rng, extra, pool=None):
@@ -231,10 +278,12 @@ def run_gpu_ex(ctx: int, pr: Prepared, which=("rr", "hrr", "cp", "rho", "psi")):
             {k: v.cpu().numpy().astype(np.float64) for k, v in bufs.items()})
 
 
-def check_ex(pr: Prepared, ref, ex: dict, bf16: bool, lam: float = 0.1):
+def check_ex(pr: Prepared, ref, ex: dict, bf16: bool, lam: float = 0.1, tensor_scale: float = 1.0):
     """Element-wise gates on the extra outputs, derived from the gates on Y_new and T_new (R22):
     RR_k = rho (Y_new,k - Y_k)/dt inherits tol(Y_new,k) rho/dt (+ FP32 output rounding); HRR = -sum h_k RR_k inherits
-    sum_k |h_k| tol(RR_k); cp, rho, psi move with T_new (0.5 K / 1e-3 K) and Y_new (2e-3 / 1e-5)."""
+    sum_k |h_k| tol(RR_k); cp, rho, psi move with T_new (0.5 K / 1e-3 K) and Y_new (2e-3 / 1e-5).  Those forms are as wide
+    as RR and HRR themselves on the tensor path; the gates that bite are R22' below (RR in the update's norms, HRR through
+    the tolerance on T).  tensor_scale = 2^-3 for GPUANN_PRECISION_FP16 (R23) scales the R22' gates."""
     st, th, cfg = pr.prob.state, pr.prob.thermo, pr.prob.cfg
     der = oracle.Oracle(pr.model).derived(st.T, st.p, st.Y, cfg.dt, ref)
     act = ref.flags != 4
@@ -252,12 +301,20 @@ def check_ex(pr: Prepared, ref, ex: dict, bf16: bool, lam: float = 0.1):
     rho_in = st.p.astype(np.float64) / (8314.46261815324 * st.T.astype(np.float64) * (Yc / th.W[:, None]).sum(axis=0))
     tolRR = rho_in / cfg.dt * (tolY + 2e-7 * np.abs(st.Y.astype(np.float64))) + 1e-5 * np.abs(der.rr)
     out = {}
+    gate = (2e-2 if bf16 else 1e-4) * tensor_scale
     if "rr" in ex:
         err = np.abs(ex["rr"] - der.rr)[:, act]
         assert np.isfinite(ex["rr"][:, act]).all()
         out["rr"] = (err / tolRR[:, act]).max()
         assert out["rr"] <= 1.0, f"RR: max err/tol = {out['rr']:.3f}"
         assert np.isnan(ex["rr"][:, ~act]).all(), "RR of a skipped cell was written"
+        # R22': RR_k = rho dY_k / dt is the update itself, so it takes the update's gate (check_Y_update) in the same two
+        # norms, per species over the batch; floor = the FP32 rounding of Y_new and Y_in (rho/dt 2e-7 |Y|) and of RR
+        floor = (rho_in / cfg.dt * 2e-7 * np.abs(st.Y.astype(np.float64)) + 1e-6 * np.abs(der.rr))[:, act]
+        r2, rm = norms_against((ex["rr"] - der.rr)[:, act], der.rr[:, act], floor, gate)
+        out["rr_update"] = max(r2, rm)
+        assert r2 <= 1.0, f"RR: per-species L2 error / allowance = {r2:.3f} (allowance = {gate:g} ||RR_ref||_2 + floor)"
+        assert rm <= 1.0, f"RR: per-species max error / allowance = {rm:.3f} (allowance = {gate:g} max|RR_ref| + floor)"
     if "hrr" in ex:
         hk = np.empty_like(Yr)
         for k in range(Yr.shape[0]):
@@ -273,6 +330,21 @@ def check_ex(pr: Prepared, ref, ex: dict, bf16: bool, lam: float = 0.1):
         out["hrr"] = (err / tolH[act]).max()
         assert out["hrr"] <= 1.0, f"HRR: max err/tol = {out['hrr']:.3f}"
         assert np.isnan(ex["hrr"][~act]).all()
+        # R22': HRR dt / rho = - sum_k h_k(T_new) dY_k = the sensible-enthalpy change ~ cp (T_new - T), so an HRR error e is
+        # a temperature error e dt / (rho cp).  Per cell it must stay inside the tolerance stated on T (0.5 K; FP32 path
+        # 1e-3 K; FP16 x 2^-3) -- tolH above sums |h_k| of terms that cancel and is 2-6 x |HRR| itself -- and over the
+        # batch ||HRR - HRR_ref||_2 <= 3e-2 ||HRR_ref||_2 (the update's 2e-2 plus the T gate's share).  The absolute floor
+        # is the FP32 rounding of the terms that cancel in the sum.
+        dT_tol = (0.5 if bf16 else 1e-3) * tensor_scale
+        floorH = (np.abs(hk) * (rho_in / cfg.dt * 2e-7 * np.abs(st.Y.astype(np.float64)) + 1e-6 * np.abs(der.rr))).sum(axis=0)
+        tolH_T = rho_in * der.cp / cfg.dt * dT_tol + floorH
+        out["hrr_T"] = (err / tolH_T[act]).max() if err.size else 0.0
+        assert out["hrr_T"] <= 1.0, f"HRR: max err / (rho cp {dT_tol:g} K / dt) = {out['hrr_T']:.3f}"
+        gH = (3e-2 if bf16 else 1e-4) * tensor_scale
+        e2 = np.sqrt((err * err).sum())
+        a2 = gH * np.sqrt((der.hrr[act] ** 2).sum()) + np.sqrt((floorH[act] ** 2).sum())
+        out["hrr_l2"] = float(e2 / a2) if a2 > 0 else (0.0 if e2 == 0 else np.inf)
+        assert out["hrr_l2"] <= 1.0, f"HRR: batch L2 error / allowance = {out['hrr_l2']:.3f} (allowance = {gH:g} ||HRR_ref||_2 + floor)"
     for name, want in (("cp", der.cp), ("rho", der.rho_new), ("psi", der.psi)):
         if name in ex:
             err = np.abs(ex[name] - want)[act] / (rel_T[act] * np.abs(want[act]))
@@ -294,4 +366,5 @@ def check_all_fp16(g: GpuResult, ref, lam: float = 0.1):
     sens = np.where(np.isfinite(sens), sens, 1.0)
     worst = (np.abs(Yg - Yr) / (2.5e-4 * sens * np.abs(Yr) + 1e-10)).max()
     assert worst <= 1.0, f"Y_new (FP16 path): max err/tol = {worst:.3f}"
-    return {"raw_l2": l2, "raw_max": mx, "dT": dT, "Y": worst, "sumY": check_sumY(g.Y_new)}
+    return {"raw_l2": l2, "raw_max": mx, "dT": dT, "Y": worst, "dY": check_Y_update(g, ref, gate=2.5e-3),
+            "sumY": check_sumY(g.Y_new)}

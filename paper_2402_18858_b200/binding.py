@@ -7,12 +7,16 @@ cannot be loaded this module raises, and `gpuann_create` fails without an sm_100
 from __future__ import annotations
 
 import ctypes as C
+import os
 from pathlib import Path
 from typing import Optional, Sequence
 
 import numpy as np
 
-_LIB_PATH = Path(__file__).resolve().parent / "libgpuann.so"
+# GPUANN_DEBUG_SPIN=1 selects the debug build (python -m paper_2402_18858_b200.build --debug), whose mbarrier waits trap
+# after 2 s instead of hanging the GPU; same ABI, same kernels otherwise
+_LIB_PATH = Path(__file__).resolve().parent / (
+    "libgpuann_debug.so" if os.environ.get("GPUANN_DEBUG_SPIN") == "1" else "libgpuann.so")
 
 GPUANN_OK = 0
 GPUANN_ERR_INVALID_ARG = 1
@@ -60,8 +64,8 @@ def lib() -> C.CDLL:
     if _lib is not None:
         return _lib
     if not _LIB_PATH.exists():
-        raise RuntimeError(f"{_LIB_PATH} is missing: run `python -m paper_2402_18858_b200.build` "
-                           "(there is no CPU fallback)")
+        raise RuntimeError(f"{_LIB_PATH} is missing: run `python -m paper_2402_18858_b200.build"
+                           f"{' --debug' if _LIB_PATH.name.endswith('_debug.so') else ''}` (there is no CPU fallback)")
     L = C.CDLL(str(_LIB_PATH))
     vp, i64, dbl = C.c_void_p, C.c_int64, C.c_double
     fpp = C.POINTER(C.POINTER(C.c_float))

@@ -67,15 +67,55 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, uint32_t parity) {
     return ok != 0;
 }
 
+// Debug build (-DGPUANN_DEBUG_SPIN; `python -m paper_2402_18858_b200.build --debug` -> libgpuann_debug.so, loaded by the
+// binding when GPUANN_DEBUG_SPIN=1 is in the environment): a wait that has been polling for more than kSpinLimitNs of
+// %globaltimer prints which barrier it is stuck on and traps.  A wrong phase or a missing arrive in a new kernel variant is
+// then a failed launch (cudaErrorLaunchFailure at the next synchronisation; the printf line is best effort) instead of a
+// GPU that hangs until the lease is killed.  compute-sanitizer is not available on this pool.
+// The release build compiles none of this.
+#ifdef GPUANN_DEBUG_SPIN
+constexpr unsigned long long kSpinLimitNs = 2000000000ull;
+__device__ __forceinline__ unsigned long long spin_now_ns() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+static __device__ __noinline__ void spin_timeout(uint32_t bar_addr, uint32_t parity, uint32_t bar_addr_b, uint32_t parity_b) {
+    printf("gpuann: mbarrier wait > 2 s: block %d thread %d (warp %d) barrier smem 0x%x parity %u%s", (int)blockIdx.x,
+           (int)threadIdx.x, (int)(threadIdx.x >> 5), bar_addr, parity, bar_addr_b ? "" : "\n");
+    if (bar_addr_b) printf(" / barrier smem 0x%x parity %u\n", bar_addr_b, parity_b);
+    __trap();
+}
+// one poll in 1024 reads the timer
+#define GPUANN_SPIN_GUARD(polls, t0, a, pa, b, pb)                                      \
+    if (((++(polls)) & 1023u) == 0) {                                                   \
+        const unsigned long long now__ = spin_now_ns();                                 \
+        if ((t0) == 0) (t0) = now__;                                                    \
+        else if (now__ - (t0) > kSpinLimitNs) spin_timeout((a), (pa), (b), (pb));        \
+    }
+#endif
+
 // Blocks until the phase with the given parity has completed.
 __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+#ifdef GPUANN_DEBUG_SPIN
+    uint32_t polls = 0;
+    unsigned long long t0 = 0;
+    while (!mbar_try_wait(bar, parity)) {
+        GPUANN_SPIN_GUARD(polls, t0, smem_u32(bar), parity, 0u, 0u)
+    }
+#else
     while (!mbar_try_wait(bar, parity)) {
     }
+#endif
 }
 
 // Blocks until both phases have completed; the two polls are issued back to back so that their latencies overlap.
 __device__ __forceinline__ void mbar_wait2(uint64_t *bar_a, uint32_t parity_a, uint64_t *bar_b, uint32_t parity_b) {
     uint32_t a, b;
+#ifdef GPUANN_DEBUG_SPIN
+    uint32_t polls = 0;
+    unsigned long long t0 = 0;
+#endif
     do {
         asm volatile(
             "{\n\t"
@@ -88,6 +128,9 @@ __device__ __forceinline__ void mbar_wait2(uint64_t *bar_a, uint32_t parity_a, u
             : "=r"(a), "=r"(b)
             : "r"(smem_u32(bar_a)), "r"(parity_a), "r"(smem_u32(bar_b)), "r"(parity_b)
             : "memory");
+#ifdef GPUANN_DEBUG_SPIN
+        GPUANN_SPIN_GUARD(polls, t0, smem_u32(bar_a), parity_a, smem_u32(bar_b), parity_b)
+#endif
     } while (!(a & b));
 }
 

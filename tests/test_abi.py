@@ -73,5 +73,15 @@ def test_no_cpu_fallback_and_null_checks(lib):
         with pytest.raises(B.GpuannError):
             B.gpuann_create()
     assert lib.gpuann_chem_step(None, 0, None, None, None, None, 1e-6, None) == B.GPUANN_ERR_INVALID_ARG
+    assert lib.gpuann_input_moments_static(None, 1, 1, None, None, None, 0.1, None, None, None) == B.GPUANN_ERR_INVALID_ARG
     assert lib.gpuann_destroy(None) == B.GPUANN_OK
     assert lib.gpuann_launch_count(None) == 0
+
+
+def test_static_scratch_limits_match_the_header():
+    """GPUANN_STATIC_MAX_SPECIES / GPUANN_STATIC_SCRATCH_BYTES: header, binding and the layout the header states
+    ((512 blocks x (64 + 2) features + 2 x 66) doubles) agree; k_aux.cu static_asserts the same two numbers."""
+    hdr = {m.group(1): int(m.group(2)) for m in re.finditer(r"#define (GPUANN_STATIC_\w+) (\d+)", HEADER)}
+    assert hdr == {"GPUANN_STATIC_MAX_SPECIES": B.GPUANN_STATIC_MAX_SPECIES, "GPUANN_STATIC_SCRATCH_BYTES": B.GPUANN_STATIC_SCRATCH_BYTES}
+    d = B.GPUANN_STATIC_MAX_SPECIES + 2
+    assert B.GPUANN_STATIC_SCRATCH_BYTES == (512 * d + 2 * d) * 8

@@ -85,3 +85,13 @@ def test_static_scratch_limits_match_the_header():
     assert hdr == {"GPUANN_STATIC_MAX_SPECIES": B.GPUANN_STATIC_MAX_SPECIES, "GPUANN_STATIC_SCRATCH_BYTES": B.GPUANN_STATIC_SCRATCH_BYTES}
     d = B.GPUANN_STATIC_MAX_SPECIES + 2
     assert B.GPUANN_STATIC_SCRATCH_BYTES == (512 * d + 2 * d) * 8
+
+
+def test_debug_library_has_the_same_abi():
+    """libgpuann_debug.so (build.py --debug: -DGPUANN_DEBUG_SPIN) exports every symbol the header declares; skipped when
+    it has not been built (__graft_entry__.build() builds it)."""
+    if not BUILD.LIB_DEBUG.exists() or BUILD.needs_build(BUILD.LIB_DEBUG):
+        pytest.skip("libgpuann_debug.so not built or out of date")
+    dbg = C.CDLL(str(BUILD.LIB_DEBUG))
+    for name in declared_symbols():
+        assert hasattr(dbg, name), f"libgpuann_debug.so does not export {name}"
